@@ -1,0 +1,159 @@
+"""ctypes loader for the CPU oracle (oracle/pt_oracle.cpp).  TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import this module.
+It never imports the CUDA package and the CUDA package never imports it.
+
+`prec` selects the instantiation: "f64" (double, the timed CPU baseline) or "f128" (__float128, the parity arbiter;
+results are rounded to double on return).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+import threading
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "pt_oracle.cpp")
+_LIB = os.path.join(_HERE, "libpt_oracle.so")
+_lock = threading.Lock()
+_lib = None
+
+PREC = {"f64": 0, "f128": 1}
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with g++ (no FMA contraction: the phase fold and subsample time are pinned IEEE ops)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".tmp%d" % os.getpid()
+        cmd = ["g++", "-O2", "-std=gnu++17", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", _SRC, "-o", tmp,
+               "-lquadmath"]
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def lib() -> C.CDLL:
+    global _lib
+    with _lock:
+        if _lib is None:
+            _lib = C.CDLL(build())
+            for name in ("pto_ma_basis", "pto_ellip", "pto_kepler", "pto_orbit_z", "pto_ma_quad_exact",
+                         "pto_ma_table_build", "pto_ma_quad_interp", "pto_num_threads"):
+                getattr(_lib, name).restype = C.c_int
+            _lib.pto_set_num_threads.restype = None
+    return _lib
+
+
+def _p(a: np.ndarray):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _f64(a) -> np.ndarray:
+    return np.ascontiguousarray(np.asarray(a, dtype=np.float64))
+
+
+def num_threads() -> int:
+    return int(lib().pto_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    lib().pto_set_num_threads(C.c_int(int(n)))
+
+
+def ma_basis(k, z, prec: str = "f128"):
+    """λe, λd*, ηd at matching arrays of radius ratio k and separation z."""
+    k, z = np.broadcast_arrays(_f64(k), _f64(z))
+    k, z = _f64(k), _f64(z)
+    out = [np.empty(k.shape, np.float64) for _ in range(3)]
+    rc = lib().pto_ma_basis(C.c_int(PREC[prec]), _p(k), _p(z), C.c_int64(k.size), *[_p(o) for o in out])
+    assert rc == 0
+    return tuple(out)
+
+
+def ellip(m, n, prec: str = "f128"):
+    """K(m), E(m), Π(n|m) — parameter form, minus-sign convention for n."""
+    m, n = np.broadcast_arrays(_f64(m), _f64(n))
+    m, n = _f64(m), _f64(n)
+    out = [np.empty(m.shape, np.float64) for _ in range(3)]
+    rc = lib().pto_ellip(C.c_int(PREC[prec]), _p(m), _p(n), C.c_int64(m.size), *[_p(o) for o in out])
+    assert rc == 0
+    return tuple(out)
+
+
+def kepler(M, e, prec: str = "f128"):
+    M, e = np.broadcast_arrays(_f64(M), _f64(e))
+    M, e = _f64(M), _f64(e)
+    E = np.empty(M.shape, np.float64)
+    rc = lib().pto_kepler(C.c_int(PREC[prec]), _p(M), _p(e), C.c_int64(M.size), _p(E))
+    assert rc == 0
+    return E
+
+
+def _shape_args(times, params, n_pb):
+    times = _f64(times)
+    params = _f64(params)
+    if params.ndim == 1:
+        params = params[None, :]
+    n_pv = params.shape[0]
+    assert params.shape[1] == 6 + 3 * n_pb, "parameter row must hold 6 + 3*n_pb doubles"
+    if times.ndim == 1:
+        n_t, stride = times.shape[0], 0
+    else:
+        assert times.shape[0] == n_pv
+        n_t, stride = times.shape[1], times.shape[1]
+    return times, params, n_pv, n_t, stride
+
+
+def orbit_z(times, params, n_pb: int = 1, n_ss: int = 1, t_exp: float = 0.0, prec: str = "f128"):
+    """Signed projected separation [n_pv][n_t][n_ss]; negative = planet behind the star."""
+    times, params, n_pv, n_t, stride = _shape_args(times, params, n_pb)
+    z = np.empty((n_pv, n_t, n_ss), np.float64)
+    rc = lib().pto_orbit_z(C.c_int(PREC[prec]), _p(times), C.c_int64(n_t), C.c_int64(stride), _p(params),
+                           C.c_int64(n_pv), C.c_int32(n_pb), C.c_int32(n_ss), C.c_double(t_exp), _p(z))
+    assert rc == 0, rc
+    return z
+
+
+def ma_quad_exact(times, params, n_pb: int = 1, n_ss: int = 1, t_exp: float = 0.0, prec: str = "f128"):
+    """Relative flux [n_pv][n_pb][n_t] of the exact quadratic Mandel–Agol model."""
+    times, params, n_pv, n_t, stride = _shape_args(times, params, n_pb)
+    f = np.empty((n_pv, n_pb, n_t), np.float64)
+    rc = lib().pto_ma_quad_exact(C.c_int(PREC[prec]), _p(times), C.c_int64(n_t), C.c_int64(stride), _p(params),
+                                 C.c_int64(n_pv), C.c_int32(n_pb), C.c_int32(n_ss), C.c_double(t_exp), _p(f))
+    assert rc == 0, rc
+    return f
+
+
+def table_spacing(k_min: float, k_max: float, n_k: int, z_max: float, n_z: int):
+    """(dk, dz) exactly as the table builder forms them (IEEE double)."""
+    return (np.float64(k_max) - np.float64(k_min)) / np.float64(n_k - 1), np.float64(z_max) / np.float64(n_z - 1)
+
+
+def ma_table_build(k_min, k_max, n_k, z_max, n_z, dtype=np.float64, n_fn: int = 3, prec: str = "f128"):
+    """(k,z) table [n_k][n_z][n_fn] of λe, λd*, ηd(, 0)."""
+    dtype = np.dtype(dtype)
+    code = {np.dtype(np.float64): 0, np.dtype(np.float32): 1}[dtype]
+    tb = np.zeros((n_k, n_z, n_fn), dtype)
+    rc = lib().pto_ma_table_build(C.c_int(PREC[prec]), C.c_double(k_min), C.c_double(k_max), C.c_int32(n_k),
+                                  C.c_double(z_max), C.c_int32(n_z), C.c_int32(code), C.c_int32(n_fn), _p(tb))
+    assert rc == 0, rc
+    return tb
+
+
+def ma_quad_interp(table, k_min, dk, dz, times, params, n_pb: int = 1, n_ss: int = 1, t_exp: float = 0.0,
+                   prec: str = "f128"):
+    """Relative flux [n_pv][n_pb][n_t] by bilinear interpolation of `table`."""
+    table = np.ascontiguousarray(table)
+    code = {np.dtype(np.float64): 0, np.dtype(np.float32): 1}[table.dtype]
+    n_k, n_z, n_fn = table.shape
+    times, params, n_pv, n_t, stride = _shape_args(times, params, n_pb)
+    f = np.empty((n_pv, n_pb, n_t), np.float64)
+    rc = lib().pto_ma_quad_interp(C.c_int(PREC[prec]), _p(table), C.c_int32(code), C.c_int32(n_k), C.c_int32(n_z),
+                                  C.c_int32(n_fn), C.c_double(k_min), C.c_double(dk), C.c_double(dz), _p(times),
+                                  C.c_int64(n_t), C.c_int64(stride), _p(params), C.c_int64(n_pv), C.c_int32(n_pb),
+                                  C.c_int32(n_ss), C.c_double(t_exp), _p(f))
+    assert rc == 0, rc
+    return f
