@@ -1,0 +1,119 @@
+/* pt.h — C ABI of the B200-native batched quadratic Mandel–Agol transit-model evaluator.
+ *
+ * The method is the one PyTransit (Parviainen 2015, arXiv 1504.07433) implements; "P:Ln" cites line n of the paper's
+ * text, DESIGN.md §2 lists the readings taken where the paper is silent or garbled.
+ *
+ *   flux  f(k,z) = 1 - [(1-c) λe(k,z) + c λd(k,z) + b ηd(k,z)] / (1 - a/3 - b/6),  c = a + 2b          P:L136 (Eq. 13)
+ *   (a,b) = (u1,u2): quadratic limb darkening  I(μ)/I(1) = 1 - a(1-μ) - b(1-μ)²                        P:L86  (Eq. 6)
+ *   λe, λd, ηd: Mandel & Agol (2002) basis functions, independent of limb darkening
+ *   "λd" is the continuous function λd + (2/3)Θ(k-z) (Eq. 13 prints no Θ term; R3)
+ *
+ * Conventions common to every entry point
+ *   - Pointers named d_* are DEVICE pointers (e.g. torch tensor .data_ptr()); pointers named h_* are HOST pointers.
+ *     The caller owns all of them.  The d_* entry points never allocate, free, copy to the host or synchronise: they
+ *     validate their arguments, enqueue kernels on `stream` (a cudaStream_t passed as void*; NULL = default stream)
+ *     and return.  They hold no global state and are re-entrant.
+ *   - Parameter rows (`d_params`, row-major [n_pv][6 + 3 n_pb] doubles):
+ *         [ t0, P, a/R*, i, e, w,  k_0, u1_0, u2_0,  k_1, u1_1, u2_1, ... ]
+ *     t0 = time of inferior conjunction, P = period (same unit as the times), a/R* = scaled semi-major axis,
+ *     i = inclination and w = argument of periastron in RADIANS, e = eccentricity in [0,1), per passband j the
+ *     radius ratio k_j = R_planet/R_star and the two limb-darkening coefficients.  n_pb = 1 is the 9-vector
+ *     [t0,P,a/R*,i,e,w,k,u1,u2].  The orbit equations are not in the paper (P:L31 names the solvers): standard
+ *     two-body projection, observer on +Z, transit at true anomaly π/2 - w (R5); e == 0 selects the circular
+ *     routine, e > 0 the Newton–Kepler solver ("selects the most appropriate orbit calculation routine based on
+ *     the eccentricity").
+ *   - Times: `d_times` holds n_t doubles shared by all parameter vectors when t_stride_pv == 0, else row pv starts at
+ *     d_times + pv * t_stride_pv (t_stride_pv >= n_t).
+ *   - Supersampling: every exposure is the mean of n_ss model values at the midpoints of n_ss equal
+ *     sub-intervals of [t - t_exp/2, t + t_exp/2]; n_ss == 1 ignores t_exp.
+ *   - Multi-passband: the basis functions are evaluated once per sample at the mean radius ratio
+ *     k̂ = (1/n_pb) Σ k_j and combined per passband; each passband's flux decrement is scaled by k_j²/k̂².
+ *   - Planet behind the star, z >= 1 + k̂, or k̂ == 0  =>  flux = 1 exactly.
+ *   - Return value: PT_OK, or a synchronous argument error (nothing is enqueued or written in that case).
+ *     Data errors are asynchronous: a parameter row with a non-finite entry, P <= 0, a/R* <= 0, e outside [0,1), any
+ *     k_j < 0 or 1 - u1_j/3 - u2_j/6 == 0 gets its whole output row set to NaN; if d_status != NULL,
+ *     PT_ST_BAD_PARAM is OR-ed into d_status[0] and d_status[1] is incremented once per affected row.
+ *     d_status (2 x int32) is only ever OR-ed/incremented: the caller zeroes it.
+ */
+#ifndef PT_H_
+#define PT_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { PT_OK = 0, PT_ERR_NULL = 1, PT_ERR_SIZE = 2, PT_ERR_DTYPE = 3, PT_ERR_TABLE = 4, PT_ERR_CUDA = 5 };
+enum { PT_F64 = 0, PT_F32 = 1 };                          /* arithmetic + storage type of the flux / of a table */
+enum { PT_ST_BAD_PARAM = 1, PT_ST_K_OUT_OF_TABLE = 2 };   /* bits OR-ed into d_status[0] */
+
+/* Interpolation table descriptor (host struct holding a device pointer).  Layout [n_k][n_z][n_fn], n_fn = 3
+ * (λe, λd, ηd) or 4 (padded with 0); node (i,j) sits at k = k_min + i*dk, z = j*dz (R10). */
+typedef struct pt_table {
+  const void* d_data;
+  int32_t dtype;      /* PT_F64 or PT_F32 storage; values are converted on load */
+  int32_t n_k, n_z, n_fn;
+  double k_min, dk, dz;
+} pt_table;
+
+/* Version / build information: returns the compute capability the kernels were built for (100 => sm_100a). */
+int pt_build_arch(void);
+
+/* S1-S2 of the hot path: projected separation of every subsample (P:L31 orbit utilities).
+ *   d_z [n_pv][n_t][n_ss] doubles; the sign carries the side: +z planet in front of the star, -z behind it.
+ *   Rows with bad parameters are NaN.  n_pb is only needed for the row length. */
+int pt_orbit_z(const double* d_times, int64_t n_t, int64_t t_stride_pv, const double* d_params, int64_t n_pv,
+               int32_t n_pb, int32_t n_ss, double t_exp, double* d_z, void* stream);
+
+/* S0-S7: exact quadratic Mandel–Agol flux (Eq. 13 with P:L143).
+ *   dtype  PT_F64: all arithmetic fp64, d_flux is double.  PT_F32: time -> phase -> z in fp64, the case split, basis
+ *          functions and combine in fp32 (fp64 only where fp32 cannot hold 2e-6, H5), d_flux is float.
+ *   d_flux [n_pv][n_pb][n_t], time fastest.   d_status: NULL or 2 x int32 (see above). */
+int pt_ma_quad_exact(const double* d_times, int64_t n_t, int64_t t_stride_pv, const double* d_params, int64_t n_pv,
+                     int32_t n_pb, int32_t n_ss, double t_exp, int32_t dtype, void* d_flux, int32_t* d_status,
+                     void* stream);
+
+/* S8: build the (k,z) interpolation table ("precomputed into two-dimensional interpolation tables spanning
+ * z = [0..1+k] and k ranges based on the prior set on k").
+ *   node (i,j): k = k_min + i*dk, dk = (k_max-k_min)/(n_k-1);  z = j*dz, dz = z_max/(n_z-1)  (IEEE double, mul then add).
+ *   Values are computed in fp64 and stored as `dtype`; d_table [n_k][n_z][n_fn], n_fn in {3,4}.
+ *   Requires n_k >= 2, n_z >= 2, 0 <= k_min < k_max, z_max > 0. */
+int pt_ma_table_build(double k_min, double k_max, int32_t n_k, double z_max, int32_t n_z, int32_t dtype, int32_t n_fn,
+                      void* d_table, void* stream);
+
+/* S9 (+S0-S3, S6, S7): interpolated quadratic Mandel–Agol flux ("bilinear interpolation"):
+ *   rk = (k̂-k_min)/dk, ik = min(floor(rk), n_k-2), fk = rk-ik; rz = z/dz, iz = min(floor(rz), n_z-2), fz = rz-iz;
+ *   v = (1-fk)[(1-fz)T[ik][iz] + fz T[ik][iz+1]] + fk[(1-fz)T[ik+1][iz] + fz T[ik+1][iz+1]] for each function, then
+ *   Eq. 13.  Samples with z >= 1+k̂ never touch the table.  `dtype` is the arithmetic/output type as above; the table's
+ *   own storage type is in the descriptor.  A parameter vector whose k̂ lies outside [k_min, k_min+(n_k-1)dk] is
+ *   evaluated by the exact device path and PT_ST_K_OUT_OF_TABLE is raised (paper silent; R13).
+ *   PT_ERR_TABLE: descriptor inconsistent (NULL data, n_k/n_z < 2, n_fn not 3/4, dk/dz <= 0, unknown dtype). */
+int pt_ma_quad_interp(const pt_table* table, const double* d_times, int64_t n_t, int64_t t_stride_pv,
+                      const double* d_params, int64_t n_pv, int32_t n_pb, int32_t n_ss, double t_exp, int32_t dtype,
+                      void* d_flux, int32_t* d_status, void* stream);
+
+/* Host-buffer convenience forms (the end-to-end path of P:L173/P:L198: copy inputs to the GPU, evaluate, copy the
+ * flux back).  All pointers are HOST pointers (pinned memory makes the copies asynchronous); the call allocates
+ * stream-ordered scratch on the current device, enqueues H2D copies, the same kernels as above and the D2H copy on an
+ * internal stream, and returns after that stream has drained.  h_status: NULL or 2 x int32, overwritten.
+ * pt_ma_quad_interp_host takes the table as a descriptor whose d_data is still a DEVICE pointer (tables are built once
+ * and stay resident). */
+int pt_ma_quad_exact_host(const double* h_times, int64_t n_t, int64_t t_stride_pv, const double* h_params, int64_t n_pv,
+                          int32_t n_pb, int32_t n_ss, double t_exp, int32_t dtype, void* h_flux, int32_t* h_status);
+int pt_ma_quad_interp_host(const pt_table* table, const double* h_times, int64_t n_t, int64_t t_stride_pv,
+                           const double* h_params, int64_t n_pv, int32_t n_pb, int32_t n_ss, double t_exp,
+                           int32_t dtype, void* h_flux, int32_t* h_status);
+
+/* Diagnostics for the roofline denominator (the FP64 vector-pipe peak is not in MEASURED_PEAKS.json):
+ * every thread of `blocks` x 256 runs `iters` rounds of 8 independent DFMA chains and stores one double to
+ * d_sink[blocks*256] so the work cannot be removed.  FP64 thread-instructions issued = blocks*256*iters*8. */
+int pt_probe_dfma(int32_t blocks, int32_t iters, double* d_sink, void* stream);
+
+/* Number of kernel launches the library has enqueued so far in this process (bench.py's gpu_launches evidence). */
+int64_t pt_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PT_H_ */

@@ -1,0 +1,188 @@
+"""Thin Python binding of the C ABI in include/pt.h: argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of libpt_b200.so; PyTorch is used for device memory and streams.
+There is no CPU fallback: importing works without a GPU (so that the symbol table can be checked), but loading fails
+loudly if the shared library has not been built, and every compute call requires CUDA tensors.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpt_b200.so")
+
+PT_OK, PT_ERR_NULL, PT_ERR_SIZE, PT_ERR_DTYPE, PT_ERR_TABLE, PT_ERR_CUDA = range(6)
+PT_F64, PT_F32 = 0, 1
+PT_ST_BAD_PARAM, PT_ST_K_OUT_OF_TABLE = 1, 2
+_ERR = {1: "PT_ERR_NULL", 2: "PT_ERR_SIZE", 3: "PT_ERR_DTYPE", 4: "PT_ERR_TABLE", 5: "PT_ERR_CUDA"}
+
+EXPORTS = ("pt_build_arch", "pt_orbit_z", "pt_ma_quad_exact", "pt_ma_table_build", "pt_ma_quad_interp",
+           "pt_ma_quad_exact_host", "pt_ma_quad_interp_host", "pt_probe_dfma", "pt_launch_count")
+
+
+class PtError(RuntimeError):
+    pass
+
+
+class pt_table(C.Structure):
+    _fields_ = [("d_data", C.c_void_p), ("dtype", C.c_int32), ("n_k", C.c_int32), ("n_z", C.c_int32),
+                ("n_fn", C.c_int32), ("k_min", C.c_double), ("dk", C.c_double), ("dz", C.c_double)]
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load libpt_b200.so (built in-tree by paper_1504_07433_b200.build); raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise PtError("CUDA extension %s is missing: run `python -m paper_1504_07433_b200.build` "
+                          "(there is no CPU fallback)" % LIB_PATH)
+        L = C.CDLL(LIB_PATH)
+        i32, i64, dbl, ptr = C.c_int32, C.c_int64, C.c_double, C.c_void_p
+        common = [ptr, i64, i64, ptr, i64, i32, i32, dbl]
+        L.pt_build_arch.restype = C.c_int
+        L.pt_launch_count.restype = i64
+        L.pt_orbit_z.argtypes = common + [ptr, ptr]
+        L.pt_ma_quad_exact.argtypes = common + [i32, ptr, ptr, ptr]
+        L.pt_ma_table_build.argtypes = [dbl, dbl, i32, dbl, i32, i32, i32, ptr, ptr]
+        L.pt_ma_quad_interp.argtypes = [C.POINTER(pt_table)] + common + [i32, ptr, ptr, ptr]
+        L.pt_ma_quad_exact_host.argtypes = common + [i32, ptr, ptr]
+        L.pt_ma_quad_interp_host.argtypes = [C.POINTER(pt_table)] + common + [i32, ptr, ptr]
+        L.pt_probe_dfma.argtypes = [i32, i32, ptr, ptr]
+        for n in EXPORTS[1:-1]:
+            getattr(L, n).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, what: str) -> None:
+    if rc != PT_OK:
+        raise PtError("%s failed: %s" % (what, _ERR.get(rc, rc)))
+
+
+def _stream() -> int:
+    return torch.cuda.current_stream().cuda_stream
+
+
+def _dtype_code(dtype: torch.dtype) -> int:
+    if dtype == torch.float64:
+        return PT_F64
+    if dtype == torch.float32:
+        return PT_F32
+    raise PtError("flux/table dtype must be float64 or float32")
+
+
+def _marshal(times: torch.Tensor, params: torch.Tensor, n_pb: int, device_required: bool = True):
+    if params.dim() == 1:
+        params = params[None, :]
+    if times.dtype != torch.float64 or params.dtype != torch.float64:
+        raise PtError("times and params must be float64")
+    if not (times.is_contiguous() and params.is_contiguous()):
+        raise PtError("times and params must be contiguous")
+    if device_required and not (times.is_cuda and params.is_cuda):
+        raise PtError("times and params must be CUDA tensors (there is no CPU path)")
+    if not device_required and (times.is_cuda or params.is_cuda):
+        raise PtError("the *_host entry points take host tensors")
+    n_pv = params.shape[0]
+    if params.shape[1] != 6 + 3 * n_pb:
+        raise PtError("parameter rows must hold 6 + 3*n_pb doubles")
+    if times.dim() == 1:
+        n_t, stride = times.shape[0], 0
+    elif times.dim() == 2 and times.shape[0] == n_pv:
+        n_t, stride = times.shape[1], times.shape[1]
+    else:
+        raise PtError("times must be [n_t] or [n_pv][n_t]")
+    return times, params, n_pv, n_t, stride
+
+
+def pt_orbit_z(times: torch.Tensor, params: torch.Tensor, n_pb: int = 1, n_ss: int = 1, t_exp: float = 0.0,
+               out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """Signed projected separation [n_pv][n_t][n_ss] (include/pt.h: pt_orbit_z)."""
+    times, params, n_pv, n_t, stride = _marshal(times, params, n_pb)
+    if out is None:
+        out = torch.empty((n_pv, n_t, n_ss), dtype=torch.float64, device=times.device)
+    _check(lib().pt_orbit_z(times.data_ptr(), n_t, stride, params.data_ptr(), n_pv, n_pb, n_ss, float(t_exp),
+                            out.data_ptr(), _stream()), "pt_orbit_z")
+    return out
+
+
+def pt_ma_quad_exact(times: torch.Tensor, params: torch.Tensor, n_pb: int = 1, n_ss: int = 1, t_exp: float = 0.0,
+                     dtype: torch.dtype = torch.float64, out: Optional[torch.Tensor] = None,
+                     status: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """Exact quadratic Mandel–Agol flux [n_pv][n_pb][n_t] (include/pt.h: pt_ma_quad_exact)."""
+    times, params, n_pv, n_t, stride = _marshal(times, params, n_pb)
+    if out is None:
+        out = torch.empty((n_pv, n_pb, n_t), dtype=dtype, device=times.device)
+    _check(lib().pt_ma_quad_exact(times.data_ptr(), n_t, stride, params.data_ptr(), n_pv, n_pb, n_ss, float(t_exp),
+                                  _dtype_code(out.dtype), out.data_ptr(),
+                                  status.data_ptr() if status is not None else None, _stream()), "pt_ma_quad_exact")
+    return out
+
+
+class Table:
+    """A device-resident (k,z) table plus its descriptor (include/pt.h: pt_table)."""
+
+    def __init__(self, data: torch.Tensor, k_min: float, dk: float, dz: float):
+        self.data, self.k_min, self.dk, self.dz = data, float(k_min), float(dk), float(dz)
+        n_k, n_z, n_fn = data.shape
+        self.desc = pt_table(data.data_ptr(), _dtype_code(data.dtype), n_k, n_z, n_fn, self.k_min, self.dk, self.dz)
+
+
+def pt_ma_table_build(k_min: float, k_max: float, n_k: int, z_max: float, n_z: int,
+                      dtype: torch.dtype = torch.float64, n_fn: int = 3, device="cuda") -> Table:
+    """Build the interpolation table on the device (include/pt.h: pt_ma_table_build)."""
+    data = torch.empty((n_k, n_z, n_fn), dtype=dtype, device=device)
+    _check(lib().pt_ma_table_build(float(k_min), float(k_max), n_k, float(z_max), n_z, _dtype_code(dtype), n_fn,
+                                   data.data_ptr(), _stream()), "pt_ma_table_build")
+    dk = (float(k_max) - float(k_min)) / float(n_k - 1)
+    dz = float(z_max) / float(n_z - 1)
+    return Table(data, k_min, dk, dz)
+
+
+def pt_ma_quad_interp(table: Table, times: torch.Tensor, params: torch.Tensor, n_pb: int = 1, n_ss: int = 1,
+                      t_exp: float = 0.0, dtype: torch.dtype = torch.float64, out: Optional[torch.Tensor] = None,
+                      status: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """Interpolated quadratic Mandel–Agol flux [n_pv][n_pb][n_t] (include/pt.h: pt_ma_quad_interp)."""
+    times, params, n_pv, n_t, stride = _marshal(times, params, n_pb)
+    if out is None:
+        out = torch.empty((n_pv, n_pb, n_t), dtype=dtype, device=times.device)
+    _check(lib().pt_ma_quad_interp(C.byref(table.desc), times.data_ptr(), n_t, stride, params.data_ptr(), n_pv, n_pb,
+                                   n_ss, float(t_exp), _dtype_code(out.dtype), out.data_ptr(),
+                                   status.data_ptr() if status is not None else None, _stream()), "pt_ma_quad_interp")
+    return out
+
+
+def pt_ma_quad_exact_host(times: torch.Tensor, params: torch.Tensor, out: torch.Tensor, n_pb: int = 1, n_ss: int = 1,
+                          t_exp: float = 0.0, status: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """Host buffers in, host buffer out; H2D + kernels + D2H inside the call (include/pt.h: pt_ma_quad_exact_host)."""
+    times, params, n_pv, n_t, stride = _marshal(times, params, n_pb, device_required=False)
+    _check(lib().pt_ma_quad_exact_host(times.data_ptr(), n_t, stride, params.data_ptr(), n_pv, n_pb, n_ss,
+                                       float(t_exp), _dtype_code(out.dtype), out.data_ptr(),
+                                       status.data_ptr() if status is not None else None), "pt_ma_quad_exact_host")
+    return out
+
+
+def pt_ma_quad_interp_host(table: Table, times: torch.Tensor, params: torch.Tensor, out: torch.Tensor, n_pb: int = 1,
+                           n_ss: int = 1, t_exp: float = 0.0, status: Optional[torch.Tensor] = None) -> torch.Tensor:
+    times, params, n_pv, n_t, stride = _marshal(times, params, n_pb, device_required=False)
+    _check(lib().pt_ma_quad_interp_host(C.byref(table.desc), times.data_ptr(), n_t, stride, params.data_ptr(), n_pv,
+                                        n_pb, n_ss, float(t_exp), _dtype_code(out.dtype), out.data_ptr(),
+                                        status.data_ptr() if status is not None else None), "pt_ma_quad_interp_host")
+    return out
+
+
+def pt_probe_dfma(blocks: int, iters: int, sink: torch.Tensor) -> None:
+    """FP64-pipe peak probe (include/pt.h: pt_probe_dfma); sink: CUDA float64 tensor of blocks*256 elements."""
+    if not sink.is_cuda or sink.dtype != torch.float64 or sink.numel() < blocks * 256:
+        raise PtError("sink must be a CUDA float64 tensor of at least blocks*256 elements")
+    _check(lib().pt_probe_dfma(blocks, iters, sink.data_ptr(), _stream()), "pt_probe_dfma")
+
+
+def pt_launch_count() -> int:
+    return int(lib().pt_launch_count())

@@ -1,0 +1,161 @@
+// pt_basis.cuh — device implementation of the three Mandel–Agol basis functions λe, λd*, ηd in fp64.
+//
+// Formulation: the closed forms of Mandel & Agol (2002), rearranged so that no sub-expression is formed
+// by cancellation near a case boundary, with the complete elliptic integrals K, E, Π evaluated by TWO Bulirsch `cel`
+// sequences that share one AGM ladder (R. Bulirsch, Numer. Math. 13 (1969) 305: cel(kc,p,a,b) is linear in (a,b), so
+// cK·K + cE·E = cel(kc,1,cK+cE,cK+cE·mc) and Π(n|m) = cel(kc,1-n,1,1)).  The partial-overlap and planet-inside cases
+// select *coefficients*, then run the same loop, so a warp that straddles ingress does not serialise the expensive part.
+// Nothing in this file is shared with oracle/ (which uses Carlson's R_F/R_D/R_J and the textbook forms).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace pt {
+
+struct Basis {
+  double le, ld, ed;
+};
+
+constexpr double kPi = 3.14159265358979323846;
+constexpr double kInvPi = 0.31830988618379067154;
+constexpr double kTwoThirds = 0.66666666666666666667;
+
+// cK·K(m) + cE·E(m) + cP·cel(kc, 1-n, a2, b2n) with mc = 1-m = kc² and sp = sqrt(1-n) > 0 the square root of the second
+// sequence's p-argument.  (a2, b2n) = (1, 1) makes the second integral Π(n|m); (0, n) makes it Π(n|m) - K(m).
+__device__ __forceinline__ double cel_pair(double mc, double sp, double cK, double cE, double cP, double a2, double b2n) {
+  double qc = sqrt(mc);
+  // sequence 1 (p = 1): its p-iterate equals the ladder's `em`, and e/p equals the previous qc, so it needs 1/em only
+  double a1 = cK + cE;
+  double b1 = fma(cE, mc, cK);
+  // sequence 2: p2 = sqrt(1-n), b = b/p2
+  double p2 = sp;
+  double b2 = b2n / sp;
+  double e = qc, em = 1.0;
+#pragma unroll 1
+  for (int it = 0; it < 16; ++it) {
+    const double rem = 1.0 / em;
+    const double rp2 = 1.0 / p2;
+    // sequence 1
+    double f = a1;
+    a1 = fma(b1, rem, a1);
+    b1 = fma(f, qc, b1);
+    b1 += b1;
+    // sequence 2
+    f = a2;
+    a2 = fma(b2, rp2, a2);
+    const double g2 = e * rp2;
+    b2 = fma(f, g2, b2);
+    b2 += b2;
+    p2 += g2;
+    // ladder
+    const double g = em;
+    em += qc;
+    if (fabs(g - qc) <= 1.0e-8 * g) break;
+    qc = sqrt(e);
+    qc += qc;
+    e = qc * em;
+  }
+  const double s1 = fma(a1, em, b1) / (2.0 * em * em);
+  const double s2 = fma(a2, em, b2) / (em * (em + p2));
+  return (0.5 * kPi) * fma(cP, s2, s1);
+}
+
+// Basis functions at radius ratio p > 0 and separation z >= 0 (planet in front of the star).
+__device__ __forceinline__ Basis ma_basis(double p, double z) {
+  Basis r;
+  // d = z-p, s = z+p and the four contact distances 1-d, 1+d, s-1, s+1.  Each is formed so that the operand pair that
+  // nearly cancels at "its" contact is subtracted exactly first (Sterbenz), e.g. s-1 = z + (p-1) for p in [1/2, 2]:
+  // a plain (z+p)-1 loses z entirely when z << p ~ 1 (and mc = (s-1)(s+1)/(4zp) then has O(1) relative error).
+  const double d = z - p, s = z + p;
+  const double pm1 = p - 1.0;
+  const bool pmid = (p >= 0.5) & (p <= 2.0);
+  const double sm1 = pmid ? z + pm1 : (p < 0.5 ? (z - 1.0) + p : s - 1.0);   // s - 1
+  const double opd = pmid ? z - pm1 : 1.0 + d;                               // 1 + d
+  const double omd = (p < 1.0) ? (1.0 - z) + p : 1.0 - d;                    // 1 - d
+  const double sp1 = s + 1.0;
+  if (omd <= 0.0) { r.le = 0.0; r.ld = 0.0; r.ed = 0.0; return r; }                  // no overlap (z >= 1+p)
+  if (opd <= 0.0) { r.le = 1.0; r.ld = kTwoThirds; r.ed = 0.5; return r; }           // star covered (z <= p-1)
+  const double p2 = p * p, z2 = z * z;
+  const double eta2 = 0.5 * p2 * fma(2.0, z2, p2);
+  const double oma = omd * opd;                // 1 - a
+  const bool partial = sm1 > 0.0;
+
+  if (partial) {
+    const double T = sqrt(oma * sm1 * sp1);
+    const double pp1 = pm1 * (p + 1.0);                  // p² - 1 without cancellation for p ~ 1
+    const double kap0 = atan2(T, z2 + pp1);
+    const double kap1 = atan2(T, z2 - pp1);
+    r.le = (fma(p2, kap0, kap1) - 0.5 * T) * kInvPi;
+    r.ed = (fma(2.0 * eta2, kap0, kap1) - 0.25 * (1.0 + 5.0 * p2 + z2) * T) * (0.5 * kInvPi);
+  } else {
+    r.le = p2;
+    r.ed = eta2;
+  }
+
+  if (sm1 == 0.0) {  // inner contact z = 1-p: elementary closed form (exact equality only; table nodes land here)
+    r.ld = (2.0 / 3.0 * kInvPi) * acos(1.0 - 2.0 * p) - (4.0 / 9.0 * kInvPi) * (3.0 + 2.0 * p - 8.0 * p2) * sqrt(p * (1.0 - p));
+    return r;
+  }
+
+  double mc, sp, cK, cE, cP, pref, add;
+  double a2 = 1.0, b2n = 1.0;
+  if (fabs(d) < 1.0e-100) {  // z = p: the Π term drops out
+    add = 1.0 / 3.0;
+    cP = 0.0;
+    sp = 1.0;
+    if (!partial) {  // p < 1/2, m = 4p²
+      mc = (1.0 - 2.0 * p) * (1.0 + 2.0 * p);
+      cE = 4.0 * (2.0 * p2 - 1.0);
+      cK = mc;
+      pref = 2.0 / 9.0 * kInvPi;
+    } else {  // p > 1/2, m = 1/(4p²)
+      const double i4p2 = 1.0 / (4.0 * p2);
+      mc = (2.0 * p - 1.0) * (2.0 * p + 1.0) * i4p2;
+      cE = 16.0 * p * (2.0 * p2 - 1.0);
+      cK = -(1.0 - 4.0 * p2) * (3.0 - 8.0 * p2) / p;
+      pref = 1.0 / 9.0 * kInvPi;
+    }
+  } else {
+    const double rd = 1.0 / d;
+    const double q = -d * s;  // p² - z²
+    const double w7 = z2 + 7.0 * p2 - 4.0;
+    add = d < 0.0 ? kTwoThirds : 0.0;
+    cP = 3.0 * s * rd;        // -3q/a
+    if (partial) {
+      const double a = d * d, b = s * s;
+      const double pz = p * z;
+      mc = sm1 * sp1 / (4.0 * pz);
+      sp = fabs(rd);          // sqrt(1/a)
+      cE = 4.0 * pz * w7;
+      pref = (1.0 / 9.0 * kInvPi) * rsqrt(pz);
+      const double bm1 = sm1 * sp1;                      // b - 1
+      if (oma < 0.5 * a) {
+        // |n| = (1-a)/a < 1/2: write cK·K + cP·Π = (cK+cP)·K + cP·(Π-K) with cK+cP formed without cancellation.
+        // For p -> 1, z -> 0 (planet as large as the star, concentric) cK -> 3, cP -> -3, Π -> K while the prefactor
+        // 1/sqrt(pz) diverges: the plain form loses ~1e-16/sqrt(z) there.
+        cK = fma(-bm1, 2.0 * b + a - 3.0, -3.0 * q * fma(a, bm1, oma) * (rd * rd));
+        a2 = 0.0;
+        b2n = -oma * (rd * rd);                          // n = (a-1)/a
+      } else {
+        cK = fma(-bm1, 2.0 * b + a - 3.0, -3.0 * q * (b - 2.0));
+      }
+    } else {
+      mc = -sm1 * sp1 / oma;
+      sp = s * fabs(rd);      // sqrt(b/a)
+      cE = oma * w7;
+      pref = (2.0 / 9.0 * kInvPi) * rsqrt(oma);
+      const double pz4 = 4.0 * p * z;                    // b - a
+      if (pz4 < 0.5 * d * d) {
+        // |n| = (b-a)/a < 1/2: same rewrite; cK = (1-a)(1-b) + 3q, so cK + cP = (1-a)[(1-b) - 3q/a]
+        cK = oma * fma(-3.0 * q, rd * rd, -sm1 * sp1);
+        a2 = 0.0;
+        b2n = -pz4 * (rd * rd);                          // n = (a-b)/a
+      } else {
+        cK = 1.0 - 5.0 * z2 + p2 + q * q;
+      }
+    }
+  }
+  r.ld = fma(pref, cel_pair(mc, sp, cK, cE, cP, a2, b2n), add);
+  return r;
+}
+
+}  // namespace pt

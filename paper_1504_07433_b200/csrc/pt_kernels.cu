@@ -1,0 +1,493 @@
+// pt_kernels.cu — sm_100a kernels and the C ABI of include/pt.h.
+//
+// One fused kernel evaluates the whole hot path for a tile of exposures of one parameter vector:
+//   phase A  every exposure: coalesced time load, cheap phase-window test; exposures that cannot be in transit keep
+//            basis = 0 (flux exactly 1); the others are appended to a block-local queue (warp ballot + one smem atomic)
+//   phase B  dense warps drain the queue: a group of G = min(n_ss,32) lanes owns one queued exposure, each lane
+//            evaluates its subsamples (pinned fold -> orbit -> Mandel–Agol basis functions or table lookup), the group
+//            reduces λe, λd, ηd with a segmented warp shuffle and the head lane stores the means in shared memory
+//   phase C  all threads: per passband linear combine and coalesced (16-byte where aligned) stores
+// The queue is the "binning" that limits divergence: warps in phase B hold only (probably) in-transit samples, and
+// inside/partial lanes differ only in the coefficients they feed to the shared elliptic-integral loop.
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <atomic>
+
+#include "../../include/pt.h"
+#include "pt_basis.cuh"
+#include "pt_orbit.cuh"
+
+namespace pt {
+
+constexpr int kThreads = 256;
+constexpr int kTile = 1024;          // exposures per tile
+constexpr int kMaxPassbands = 1024;  // 3 doubles of shared memory each
+
+static std::atomic<int64_t> g_launches{0};
+
+struct FluxArgs {
+  const double* times;
+  int64_t n_t, t_stride_pv;
+  const double* params;
+  int64_t n_pv;
+  int n_pb, n_ss;
+  double t_exp;
+  void* flux;
+  int32_t* status;
+  int tiles_per_pv, tiles_per_block, blocks_per_pv;
+  // interpolation table (mode 1)
+  const void* tb;
+  int tb_dtype, n_k, n_z, n_fn;
+  double k_min, dk, dz, inv_dk, inv_dz;
+};
+
+__device__ __forceinline__ double nan64() { return __longlong_as_double(0x7ff8000000000000LL); }
+
+// Per-block setup: validate the row, mean radius ratio, per-passband combine coefficients, orbit constants + window.
+// coef[3*j + 0..2] = g_j (1-c_j)/N_j, g_j c_j/N_j, g_j u2_j/N_j with g_j = k_j²/k̂².
+__device__ void block_setup(PvConst& c, double* coef, const double* row, int n_pb, int n_ss, double t_exp) {
+  __shared__ int s_ok;
+  if (threadIdx.x == 0) s_ok = 1;
+  __syncthreads();
+  bool ok = true;
+  for (int j = threadIdx.x; j < n_pb; j += blockDim.x) {
+    const double k = row[6 + 3 * j], u1 = row[7 + 3 * j], u2 = row[8 + 3 * j];
+    const double N = 1.0 - u1 / 3.0 - u2 / 6.0;
+    if (!(isfinite(k) && isfinite(u1) && isfinite(u2)) || !(k >= 0.0) || N == 0.0) ok = false;
+  }
+  if (!ok) s_ok = 0;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double ksum = 0.0;
+    for (int j = 0; j < n_pb; ++j) ksum += row[6 + 3 * j];   // index order (R9)
+    c.khat = ksum / (double)n_pb;
+    pv_setup_orbit(c, row, s_ok != 0, n_ss, t_exp);
+  }
+  __syncthreads();
+  if (c.flags & PV_BAD) return;
+  const double ik2 = c.khat > 0.0 ? 1.0 / (c.khat * c.khat) : 0.0;
+  for (int j = threadIdx.x; j < n_pb; j += blockDim.x) {
+    const double k = row[6 + 3 * j], u1 = row[7 + 3 * j], u2 = row[8 + 3 * j];
+    const double cj = u1 + 2.0 * u2;
+    const double gN = k * k * ik2 / (1.0 - u1 / 3.0 - u2 / 6.0);
+    coef[3 * j + 0] = gN * (1.0 - cj);
+    coef[3 * j + 1] = gN * cj;
+    coef[3 * j + 2] = gN * u2;
+  }
+  __syncthreads();
+}
+
+// Bilinear lookup of the three functions.  Corner loads go through the read-only path; the table is
+// expected to live in L2.
+template <typename TT>
+__device__ __forceinline__ Basis table_lookup(const FluxArgs& A, int ik, double fk, double z) {
+  const double rz = z / A.dz;
+  int iz = (int)floor(rz);
+  iz = min(max(iz, 0), A.n_z - 2);
+  const double fz = rz - (double)iz;
+  const TT* r0 = (const TT*)A.tb + ((size_t)ik * A.n_z + iz) * A.n_fn;
+  const TT* r1 = r0 + (size_t)A.n_z * A.n_fn;
+  double v[3];
+#pragma unroll
+  for (int f = 0; f < 3; ++f) {
+    const double t00 = (double)__ldg(r0 + f), t01 = (double)__ldg(r0 + A.n_fn + f);
+    const double t10 = (double)__ldg(r1 + f), t11 = (double)__ldg(r1 + A.n_fn + f);
+    const double lo = fma(fz, t01 - t00, t00);
+    const double hi = fma(fz, t11 - t10, t10);
+    v[f] = fma(fk, hi - lo, lo);
+  }
+  Basis b;
+  b.le = v[0]; b.ld = v[1]; b.ed = v[2];
+  return b;
+}
+
+// MODE 0: exact.  MODE 1: interpolated (falls back to exact for a parameter vector whose k̂ is off the table).
+template <int MODE, typename OutT>
+__global__ void __launch_bounds__(kThreads, 2) flux_kernel(const FluxArgs A) {
+  extern __shared__ double s_coef[];   // 3 * n_pb
+  __shared__ PvConst c;
+  __shared__ double s_le[kTile], s_ld[kTile], s_ed[kTile];
+  __shared__ unsigned short s_queue[kTile];
+  __shared__ int s_nq;
+
+  const int64_t pv = blockIdx.x / A.blocks_per_pv;
+  const int chunk = (int)(blockIdx.x % A.blocks_per_pv);
+  const double* row = A.params + pv * (6 + 3 * (int64_t)A.n_pb);
+  const double* tt = A.times + pv * A.t_stride_pv;
+  OutT* out = (OutT*)A.flux + pv * A.n_pb * A.n_t;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+
+  block_setup(c, s_coef, row, A.n_pb, A.n_ss, A.t_exp);
+
+  const int tile_lo = chunk * A.tiles_per_block;
+  const int tile_hi = min(tile_lo + A.tiles_per_block, A.tiles_per_pv);
+  const int flags = c.flags;
+
+  if (flags & PV_BAD) {
+    const int64_t e_lo = (int64_t)tile_lo * kTile, e_hi = min((int64_t)tile_hi * kTile, A.n_t);
+    for (int j = 0; j < A.n_pb; ++j)
+      for (int64_t e = e_lo + tid; e < e_hi; e += kThreads) out[j * A.n_t + e] = (OutT)nan64();
+    if (chunk == 0 && tid == 0 && A.status) {
+      atomicOr(&A.status[0], PT_ST_BAD_PARAM);
+      atomicAdd(&A.status[1], 1);
+    }
+    return;
+  }
+
+  bool use_table = false;
+  int ik = 0;
+  double fk = 0.0;
+  if (MODE == 1) {
+    const double rk = (c.khat - A.k_min) / A.dk;
+    use_table = (c.khat >= A.k_min) && (c.khat <= A.k_min + (A.n_k - 1) * A.dk);
+    ik = min(max((int)floor(rk), 0), A.n_k - 2);
+    fk = rk - (double)ik;
+    if (!use_table && !(flags & PV_NEVER) && chunk == 0 && tid == 0 && A.status) {
+      atomicOr(&A.status[0], PT_ST_K_OUT_OF_TABLE);
+      atomicAdd(&A.status[1], 1);
+    }
+  }
+
+  // lane -> (slot, g): G lanes per queued exposure, EPW exposures per warp pass
+  const int n_ss = A.n_ss;
+  const int G = n_ss < 32 ? n_ss : 32;
+  const int EPW = 32 / G;
+  const int slot = lane / G, g = lane - slot * G;
+  const bool lane_used = slot < EPW;
+  const double off0 = (n_ss > 1) ? subsample_offset(g, n_ss, A.t_exp) : 0.0;
+  const double inv_nss = 1.0 / (double)n_ss;
+  const double khat = c.khat;
+  const double ex_lo = c.ex_lo, ex_hi = c.ex_hi;
+
+  for (int tile = tile_lo; tile < tile_hi; ++tile) {
+    const int64_t e0 = (int64_t)tile * kTile;
+    const int n_e = (int)min((int64_t)kTile, A.n_t - e0);
+    if (tid == 0) s_nq = 0;
+    __syncthreads();
+
+    // ---- phase A: window test, queue build
+    if (!(flags & PV_NEVER)) {
+      for (int i = tid; i < kTile; i += kThreads) {
+        bool inw = false;
+        if (i < n_e) {
+          s_le[i] = 0.0; s_ld[i] = 0.0; s_ed[i] = 0.0;
+          inw = (flags & PV_ALWAYS) ? true : in_window(c, __ldg(tt + e0 + i), ex_lo, ex_hi);
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, inw);
+        if (m) {
+          int base = 0;
+          if (lane == 0) base = atomicAdd(&s_nq, __popc(m));
+          base = __shfl_sync(0xffffffffu, base, 0);
+          if (inw) s_queue[base + __popc(m & ((1u << lane) - 1u))] = (unsigned short)i;
+        }
+      }
+    }
+    __syncthreads();
+    const int nq = s_nq;
+
+    // ---- phase B: drain the queue with dense warps
+    for (int q0 = warp * EPW; q0 < nq; q0 += (kThreads / 32) * EPW) {
+      const int qi = q0 + slot;
+      const bool act = lane_used && qi < nq;
+      double ale = 0.0, ald = 0.0, aed = 0.0;
+      int el = 0;
+      if (act) {
+        el = s_queue[qi];
+        const double t = __ldg(tt + e0 + el);
+        for (int s = g; s < n_ss; s += G) {
+          const double off = (s == g) ? off0 : subsample_offset(s, n_ss, A.t_exp);
+          const double ts = (n_ss > 1) ? __dadd_rn(t, off) : t;
+          const double ph = fold_phase(ts, c.t0, c.P);
+          const double zs = orbit_z_signed(c, ph);
+          if (zs >= 0.0 && zs < 1.0 + khat) {
+            Basis b;
+            if (MODE == 1 && use_table) {
+              b = (A.tb_dtype == PT_F64) ? table_lookup<double>(A, ik, fk, zs) : table_lookup<float>(A, ik, fk, zs);
+            } else {
+              b = ma_basis(khat, zs);
+            }
+            ale += b.le; ald += b.ld; aed += b.ed;
+          }
+        }
+      }
+      if (G > 1) {   // segmented sum over the G lanes of each exposure (warp-uniform branch)
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const double tle = __shfl_down_sync(0xffffffffu, ale, o);
+          const double tld = __shfl_down_sync(0xffffffffu, ald, o);
+          const double ted = __shfl_down_sync(0xffffffffu, aed, o);
+          if (g + o < G) { ale += tle; ald += tld; aed += ted; }
+        }
+      }
+      if (act && g == 0) {
+        s_le[el] = ale * inv_nss; s_ld[el] = ald * inv_nss; s_ed[el] = aed * inv_nss;
+      }
+    }
+    __syncthreads();
+
+    // ---- phase C: per-passband combine and coalesced stores
+    const bool all_one = (nq == 0);
+    // 16-byte stores: with n_t even every row start and tile start is 16-byte aligned if the base pointer is
+    const bool vec2 = (sizeof(OutT) == 8) && ((A.n_t & 1) == 0) && ((reinterpret_cast<uintptr_t>(A.flux) & 15) == 0);
+    for (int j = 0; j < A.n_pb; ++j) {
+      const double cA = s_coef[3 * j], cB = s_coef[3 * j + 1], cC = s_coef[3 * j + 2];
+      OutT* o = out + (int64_t)j * A.n_t + e0;
+      if (vec2) {
+        for (int i = 2 * tid; i < n_e; i += 2 * kThreads) {
+          double2 v;
+          if (all_one) { v.x = 1.0; v.y = 1.0; }
+          else {
+            v.x = 1.0 - fma(cC, s_ed[i], fma(cB, s_ld[i], cA * s_le[i]));
+            v.y = 1.0 - fma(cC, s_ed[i + 1], fma(cB, s_ld[i + 1], cA * s_le[i + 1]));
+          }
+          __stcs((double2*)(o + i), v);
+        }
+      } else {
+        for (int i = tid; i < n_e; i += kThreads) {
+          const double v = all_one ? 1.0 : 1.0 - fma(cC, s_ed[i], fma(cB, s_ld[i], cA * s_le[i]));
+          o[i] = (OutT)v;
+        }
+      }
+    }
+    __syncthreads();
+  }
+}
+
+// S1-S2 alone: signed projected separation of every subsample.
+__global__ void __launch_bounds__(kThreads) orbit_kernel(const double* __restrict__ times, int64_t n_t,
+                                                         int64_t t_stride_pv, const double* __restrict__ params,
+                                                         int n_pb, int n_ss, double t_exp, double* __restrict__ z_out,
+                                                         int blocks_per_pv) {
+  __shared__ PvConst c;
+  const int64_t pv = blockIdx.x / blocks_per_pv;
+  const int chunk = (int)(blockIdx.x % blocks_per_pv);
+  const double* row = params + pv * (6 + 3 * (int64_t)n_pb);
+  if (threadIdx.x == 0) {
+    bool ok = true;
+    double ksum = 0.0;
+    for (int j = 0; j < n_pb; ++j) {
+      const double k = row[6 + 3 * j], u1 = row[7 + 3 * j], u2 = row[8 + 3 * j];
+      if (!(isfinite(k) && isfinite(u1) && isfinite(u2)) || !(k >= 0.0) || (1.0 - u1 / 3.0 - u2 / 6.0) == 0.0) ok = false;
+      ksum += k;
+    }
+    c.khat = ksum / (double)n_pb;
+    pv_setup_orbit(c, row, ok, n_ss, t_exp);
+  }
+  __syncthreads();
+  const int64_t n = n_t * n_ss;
+  const double* tt = times + pv * t_stride_pv;
+  double* zo = z_out + pv * n;
+  const bool bad = c.flags & PV_BAD;
+  for (int64_t i = (int64_t)chunk * kThreads + threadIdx.x; i < n; i += (int64_t)blocks_per_pv * kThreads) {
+    double z;
+    if (bad) z = nan64();
+    else {
+      const int64_t e = i / n_ss;
+      const int s = (int)(i - e * n_ss);
+      const double t = __ldg(tt + e);
+      const double ts = (n_ss > 1) ? __dadd_rn(t, subsample_offset(s, n_ss, t_exp)) : t;
+      z = orbit_z_signed(c, fold_phase(ts, c.t0, c.P));
+    }
+    zo[i] = z;
+  }
+}
+
+// S8: table nodes.
+template <typename TT>
+__global__ void __launch_bounds__(kThreads) table_kernel(double k_min, double dk, int n_k, double dz, int n_z, int n_fn,
+                                                         TT* __restrict__ tb) {
+  const int64_t n = (int64_t)n_k * n_z;
+  for (int64_t idx = (int64_t)blockIdx.x * kThreads + threadIdx.x; idx < n; idx += (int64_t)gridDim.x * kThreads) {
+    const int i = (int)(idx / n_z), j = (int)(idx - (int64_t)i * n_z);
+    const double k = __dadd_rn(k_min, __dmul_rn((double)i, dk));
+    const double z = __dmul_rn((double)j, dz);
+    Basis b;
+    if (k > 0.0) b = ma_basis(k, z);
+    else { b.le = 0.0; b.ld = 0.0; b.ed = 0.0; }
+    TT* o = tb + idx * n_fn;
+    o[0] = (TT)b.le; o[1] = (TT)b.ld; o[2] = (TT)b.ed;
+    if (n_fn == 4) o[3] = (TT)0;
+  }
+}
+
+// FP64-pipe peak probe: 8 independent DFMA chains per thread.
+__global__ void __launch_bounds__(kThreads) dfma_probe_kernel(int iters, double* __restrict__ sink) {
+  double a0 = threadIdx.x * 1e-3, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+  const double m = 0.999999, c = 1e-6;
+#pragma unroll 4
+  for (int i = 0; i < iters; ++i) {
+    a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+    a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+  }
+  sink[(size_t)blockIdx.x * kThreads + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+}
+
+// ------------------------------------------------------------------------------------------------ host side
+static int check_common(const void* times, const void* params, const void* out, int64_t n_t, int64_t t_stride_pv,
+                        int64_t n_pv, int n_pb, int n_ss) {
+  if (!times || !params || !out) return PT_ERR_NULL;
+  if (n_t <= 0 || n_pv <= 0 || n_pb < 1 || n_ss < 1 || n_pb > kMaxPassbands) return PT_ERR_SIZE;
+  if (t_stride_pv != 0 && t_stride_pv < n_t) return PT_ERR_SIZE;
+  return PT_OK;
+}
+
+static int launch_flux(int mode, const pt_table* tb, const double* d_times, int64_t n_t, int64_t t_stride_pv,
+                       const double* d_params, int64_t n_pv, int n_pb, int n_ss, double t_exp, int dtype, void* d_flux,
+                       int32_t* d_status, cudaStream_t st) {
+  int rc = check_common(d_times, d_params, d_flux, n_t, t_stride_pv, n_pv, n_pb, n_ss);
+  if (rc) return rc;
+  if (dtype != PT_F64 && dtype != PT_F32) return PT_ERR_DTYPE;
+  FluxArgs A{};
+  A.times = d_times; A.n_t = n_t; A.t_stride_pv = t_stride_pv; A.params = d_params; A.n_pv = n_pv;
+  A.n_pb = n_pb; A.n_ss = n_ss; A.t_exp = t_exp; A.flux = d_flux; A.status = d_status;
+  if (mode == 1) {
+    if (!tb || !tb->d_data || tb->n_k < 2 || tb->n_z < 2 || (tb->n_fn != 3 && tb->n_fn != 4) || !(tb->dk > 0.0) ||
+        !(tb->dz > 0.0) || (tb->dtype != PT_F64 && tb->dtype != PT_F32))
+      return PT_ERR_TABLE;
+    A.tb = tb->d_data; A.tb_dtype = tb->dtype; A.n_k = tb->n_k; A.n_z = tb->n_z; A.n_fn = tb->n_fn;
+    A.k_min = tb->k_min; A.dk = tb->dk; A.dz = tb->dz; A.inv_dk = 1.0 / tb->dk; A.inv_dz = 1.0 / tb->dz;
+  }
+  const int64_t tiles_per_pv = (n_t + kTile - 1) / kTile;
+  if (tiles_per_pv > 0x7fffffff) return PT_ERR_SIZE;
+  const int64_t target_blocks = 148 * 8;
+  int64_t bpp = (target_blocks + n_pv - 1) / n_pv;
+  if (bpp > tiles_per_pv) bpp = tiles_per_pv;
+  if (bpp < 1) bpp = 1;
+  const int64_t tpb = (tiles_per_pv + bpp - 1) / bpp;
+  bpp = (tiles_per_pv + tpb - 1) / tpb;
+  if (n_pv * bpp > 0x7fffffff) return PT_ERR_SIZE;
+  A.tiles_per_pv = (int)tiles_per_pv; A.tiles_per_block = (int)tpb; A.blocks_per_pv = (int)bpp;
+  const dim3 grid((unsigned)(n_pv * bpp));
+  const size_t smem = (size_t)3 * n_pb * sizeof(double);
+  if (mode == 0) {
+    if (dtype == PT_F64) flux_kernel<0, double><<<grid, kThreads, smem, st>>>(A);
+    else flux_kernel<0, float><<<grid, kThreads, smem, st>>>(A);
+  } else {
+    if (dtype == PT_F64) flux_kernel<1, double><<<grid, kThreads, smem, st>>>(A);
+    else flux_kernel<1, float><<<grid, kThreads, smem, st>>>(A);
+  }
+  g_launches.fetch_add(1);
+  return cudaGetLastError() == cudaSuccess ? PT_OK : PT_ERR_CUDA;
+}
+
+}  // namespace pt
+
+using namespace pt;
+
+extern "C" {
+
+int pt_build_arch(void) {
+#ifdef PT_BUILD_ARCH
+  return PT_BUILD_ARCH;
+#else
+  return 0;
+#endif
+}
+
+int64_t pt_launch_count(void) { return g_launches.load(); }
+
+int pt_probe_dfma(int32_t blocks, int32_t iters, double* d_sink, void* stream) {
+  if (!d_sink) return PT_ERR_NULL;
+  if (blocks < 1 || iters < 1) return PT_ERR_SIZE;
+  dfma_probe_kernel<<<(unsigned)blocks, kThreads, 0, (cudaStream_t)stream>>>(iters, d_sink);
+  return cudaGetLastError() == cudaSuccess ? PT_OK : PT_ERR_CUDA;
+}
+
+int pt_orbit_z(const double* d_times, int64_t n_t, int64_t t_stride_pv, const double* d_params, int64_t n_pv,
+               int32_t n_pb, int32_t n_ss, double t_exp, double* d_z, void* stream) {
+  int rc = check_common(d_times, d_params, d_z, n_t, t_stride_pv, n_pv, n_pb, n_ss);
+  if (rc) return rc;
+  const int64_t n = n_t * n_ss;
+  int64_t bpp = (n + (int64_t)kThreads * 8 - 1) / ((int64_t)kThreads * 8);
+  const int64_t cap = (148 * 16 + n_pv - 1) / n_pv;
+  if (bpp > cap) bpp = cap;
+  if (bpp < 1) bpp = 1;
+  if (n_pv * bpp > 0x7fffffff) return PT_ERR_SIZE;
+  orbit_kernel<<<(unsigned)(n_pv * bpp), kThreads, 0, (cudaStream_t)stream>>>(d_times, n_t, t_stride_pv, d_params, n_pb,
+                                                                              n_ss, t_exp, d_z, (int)bpp);
+  g_launches.fetch_add(1);
+  return cudaGetLastError() == cudaSuccess ? PT_OK : PT_ERR_CUDA;
+}
+
+int pt_ma_quad_exact(const double* d_times, int64_t n_t, int64_t t_stride_pv, const double* d_params, int64_t n_pv,
+                     int32_t n_pb, int32_t n_ss, double t_exp, int32_t dtype, void* d_flux, int32_t* d_status,
+                     void* stream) {
+  return launch_flux(0, nullptr, d_times, n_t, t_stride_pv, d_params, n_pv, n_pb, n_ss, t_exp, dtype, d_flux, d_status,
+                     (cudaStream_t)stream);
+}
+
+int pt_ma_table_build(double k_min, double k_max, int32_t n_k, double z_max, int32_t n_z, int32_t dtype, int32_t n_fn,
+                      void* d_table, void* stream) {
+  if (!d_table) return PT_ERR_NULL;
+  if (n_k < 2 || n_z < 2 || (n_fn != 3 && n_fn != 4) || !(k_max > k_min) || !(k_min >= 0.0) || !(z_max > 0.0))
+    return PT_ERR_SIZE;
+  if (dtype != PT_F64 && dtype != PT_F32) return PT_ERR_DTYPE;
+  const double dk = (k_max - k_min) / (double)(n_k - 1), dz = z_max / (double)(n_z - 1);
+  const int64_t n = (int64_t)n_k * n_z;
+  int64_t blocks = (n + kThreads - 1) / kThreads;
+  if (blocks > 148 * 64) blocks = 148 * 64;
+  if (dtype == PT_F64)
+    table_kernel<double><<<(unsigned)blocks, kThreads, 0, (cudaStream_t)stream>>>(k_min, dk, n_k, dz, n_z, n_fn, (double*)d_table);
+  else
+    table_kernel<float><<<(unsigned)blocks, kThreads, 0, (cudaStream_t)stream>>>(k_min, dk, n_k, dz, n_z, n_fn, (float*)d_table);
+  g_launches.fetch_add(1);
+  return cudaGetLastError() == cudaSuccess ? PT_OK : PT_ERR_CUDA;
+}
+
+int pt_ma_quad_interp(const pt_table* table, const double* d_times, int64_t n_t, int64_t t_stride_pv,
+                      const double* d_params, int64_t n_pv, int32_t n_pb, int32_t n_ss, double t_exp, int32_t dtype,
+                      void* d_flux, int32_t* d_status, void* stream) {
+  return launch_flux(1, table, d_times, n_t, t_stride_pv, d_params, n_pv, n_pb, n_ss, t_exp, dtype, d_flux, d_status,
+                     (cudaStream_t)stream);
+}
+
+// ---- host-buffer forms: H2D, kernels, D2H on an internal stream, then wait.
+static int run_host(int mode, const pt_table* tb, const double* h_times, int64_t n_t, int64_t t_stride_pv,
+                    const double* h_params, int64_t n_pv, int n_pb, int n_ss, double t_exp, int dtype, void* h_flux,
+                    int32_t* h_status) {
+  int rc = check_common(h_times, h_params, h_flux, n_t, t_stride_pv, n_pv, n_pb, n_ss);
+  if (rc) return rc;
+  if (dtype != PT_F64 && dtype != PT_F32) return PT_ERR_DTYPE;
+  static thread_local cudaStream_t st = nullptr;
+  if (!st && cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) != cudaSuccess) return PT_ERR_CUDA;
+  const size_t nb_t = sizeof(double) * (size_t)(t_stride_pv == 0 ? n_t : (n_pv - 1) * t_stride_pv + n_t);
+  const size_t nb_p = sizeof(double) * (size_t)n_pv * (6 + 3 * (size_t)n_pb);
+  const size_t nb_f = (dtype == PT_F64 ? 8 : 4) * (size_t)n_pv * n_pb * n_t;
+  double *d_t = nullptr, *d_p = nullptr;
+  void* d_f = nullptr;
+  int32_t* d_s = nullptr;
+  bool ok = cudaMallocAsync(&d_t, nb_t, st) == cudaSuccess && cudaMallocAsync(&d_p, nb_p, st) == cudaSuccess &&
+            cudaMallocAsync(&d_f, nb_f, st) == cudaSuccess && cudaMallocAsync(&d_s, 8, st) == cudaSuccess;
+  if (ok) {
+    cudaMemcpyAsync(d_t, h_times, nb_t, cudaMemcpyHostToDevice, st);
+    cudaMemcpyAsync(d_p, h_params, nb_p, cudaMemcpyHostToDevice, st);
+    cudaMemsetAsync(d_s, 0, 8, st);
+    rc = launch_flux(mode, tb, d_t, n_t, t_stride_pv, d_p, n_pv, n_pb, n_ss, t_exp, dtype, d_f, d_s, st);
+    if (rc == PT_OK) {
+      cudaMemcpyAsync(h_flux, d_f, nb_f, cudaMemcpyDeviceToHost, st);
+      if (h_status) cudaMemcpyAsync(h_status, d_s, 8, cudaMemcpyDeviceToHost, st);
+    }
+  } else {
+    rc = PT_ERR_CUDA;
+  }
+  if (d_t) cudaFreeAsync(d_t, st);
+  if (d_p) cudaFreeAsync(d_p, st);
+  if (d_f) cudaFreeAsync(d_f, st);
+  if (d_s) cudaFreeAsync(d_s, st);
+  if (cudaStreamSynchronize(st) != cudaSuccess && rc == PT_OK) rc = PT_ERR_CUDA;
+  return rc;
+}
+
+int pt_ma_quad_exact_host(const double* h_times, int64_t n_t, int64_t t_stride_pv, const double* h_params, int64_t n_pv,
+                          int32_t n_pb, int32_t n_ss, double t_exp, int32_t dtype, void* h_flux, int32_t* h_status) {
+  return run_host(0, nullptr, h_times, n_t, t_stride_pv, h_params, n_pv, n_pb, n_ss, t_exp, dtype, h_flux, h_status);
+}
+
+int pt_ma_quad_interp_host(const pt_table* table, const double* h_times, int64_t n_t, int64_t t_stride_pv,
+                           const double* h_params, int64_t n_pv, int32_t n_pb, int32_t n_ss, double t_exp,
+                           int32_t dtype, void* h_flux, int32_t* h_status) {
+  return run_host(1, table, h_times, n_t, t_stride_pv, h_params, n_pv, n_pb, n_ss, t_exp, dtype, h_flux, h_status);
+}
+
+}  // extern "C"

@@ -1,0 +1,171 @@
+// pt_orbit.cuh — per-parameter-vector constants and the fused orbit stage (time -> folded phase -> projected separation).
+//
+// The paper gives no orbit equations (P:L31 only names the solvers); R5 fixes the geometry: standard two-body
+// projection, observer on +Z, t0 = time of inferior conjunction (true anomaly π/2 - w), circular routine for e == 0 and
+// Newton's method on Kepler's equation for e > 0.  Two steps are pinned to IEEE double operations (H1, H2):
+// the subsample time and the phase fold.
+#pragma once
+#include <cuda_runtime.h>
+#include <math_constants.h>
+
+namespace pt {
+
+constexpr double kTwoPi = 6.28318530717958647692;
+
+enum PvFlags : int { PV_BAD = 1, PV_CIRCULAR = 2, PV_NEVER = 4, PV_ALWAYS = 8, PV_OFF_TABLE = 16 };
+
+// Constants of one parameter vector (shared memory, one per block).
+struct PvConst {
+  double t0, P, invP;
+  double a, cosi, e, sinw, cosw, rt1me2, Mtr;
+  double khat;
+  double ph_lo, ph_hi;   // conservative phase window of the transit (cycles, relative to conjunction), sample-level
+  double ex_lo, ex_hi;   // the same widened by half an exposure: exposure-level test on the exposure centre
+  int flags;
+};
+
+// H1: phase fold — one subtraction, one IEEE division, round-to-nearest-even, one (exact) subtraction.
+__device__ __forceinline__ double fold_phase(double t, double t0, double P) {
+  const double x = __ddiv_rn(__dsub_rn(t, t0), P);
+  return __dsub_rn(x, rint(x));
+}
+
+// H2: offset of subsample s inside an exposure (midpoints of n_ss equal parts); ts = t + off, no contraction.
+__device__ __forceinline__ double subsample_offset(int s, int n_ss, double t_exp) {
+  return __dmul_rn(t_exp, __dsub_rn(__ddiv_rn((double)s + 0.5, (double)n_ss), 0.5));
+}
+
+// Cheap window test on a time: is the sample possibly in transit?  Uses t*invP (not the pinned fold) and is only ever
+// used to SKIP samples whose flux is exactly 1; the window carries a margin far above the difference between the folds.
+__device__ __forceinline__ bool in_window(const PvConst& c, double t, double lo, double hi) {
+  const double x = (t - c.t0) * c.invP;
+  const double ph = x - rint(x);
+  return ((ph > lo) & (ph < hi)) | (fabs(x) > 1.0e8);
+}
+
+// Eccentric anomaly from mean anomaly M in (-π, π] by Newton's method.  Starter: for e <= 0.8 the third-order
+// guess M + e sin M / (1 - sin(M+e) + sin M) (<= 6 steps); above that E0 = M ± e, which lies on the convex side of the
+// root so Newton descends monotonically (<= 12 steps at e = 0.999).
+__device__ __forceinline__ void kepler_newton(double M, double e, double* sinE, double* cosE) {
+  double E;
+  if (e <= 0.8) {
+    const double sM = sin(M);
+    E = M + e * sM / (1.0 - sin(M + e) + sM);
+  } else {
+    E = M + copysign(e, M);
+  }
+  double sE, cE, dE;
+  const double tol = 1.0e-9 * (1.0 - e);
+  bool conv = false;
+#pragma unroll 1
+  for (int it = 0; it < 32; ++it) {
+    sincos(E, &sE, &cE);
+    const double f = E - e * sE - M;
+    const double fp = 1.0 - e * cE;
+    dE = f / fp;
+    E -= dE;
+    if (fabs(dE) < tol) { conv = true; break; }   // the step just applied squares the error: converged to rounding
+  }
+  if (conv) {   // sin/cos of E - dE to first order in dE (|dE| < 1e-9: the neglected term is < 5e-19)
+    *sinE = fma(-cE, dE, sE);
+    *cosE = fma(sE, dE, cE);
+  } else {
+    sincos(E, sinE, cosE);
+  }
+}
+
+// Signed projected separation at pinned folded phase ph (cycles): +z in front of the star, -z behind.
+__device__ __forceinline__ double orbit_z_signed(const PvConst& c, double ph) {
+  if (c.flags & PV_CIRCULAR) {
+    double sn, cs;
+    sincospi(2.0 * ph, &sn, &cs);
+    const double cc = c.cosi * cs;
+    const double z = c.a * sqrt(fma(sn, sn, cc * cc));
+    return cs > 0.0 ? z : -z;
+  }
+  double M = fma(kTwoPi, ph, c.Mtr);
+  if (M > kPi) M -= kTwoPi;
+  if (M <= -kPi) M += kTwoPi;
+  double sE, cE;
+  kepler_newton(M, c.e, &sE, &cE);
+  const double x = cE - c.e, y = c.rt1me2 * sE;
+  const double A = c.cosw * x - c.sinw * y;   // (r/a) cos(w+f)
+  const double B = c.sinw * x + c.cosw * y;   // (r/a) sin(w+f)
+  const double Bc = B * c.cosi;
+  const double z = c.a * sqrt(fma(A, A, Bc * Bc));
+  return B > 0.0 ? z : -z;
+}
+
+// Mean anomaly of true anomaly f (any real), reduced to (-π, π].
+__device__ inline double mean_anomaly_of_true(double f, double e) {
+  double sh, ch;
+  sincos(0.5 * f, &sh, &ch);
+  const double E = 2.0 * atan2(sqrt(1.0 - e) * sh, sqrt(1.0 + e) * ch);
+  return E - e * sin(E);
+}
+
+// Validate a parameter row and fill the orbit part of PvConst (khat is set by the caller beforehand).
+// `row` = [t0, P, a/R*, i, e, w, ...]; half_exp_phase = half the exposure in cycles (0 when n_ss == 1).
+__device__ inline void pv_setup_orbit(PvConst& c, const double* row, bool row_ok, int n_ss, double t_exp) {
+  const double t0 = row[0], P = row[1], a = row[2], inc = row[3], e = row[4], w = row[5];
+  int flags = 0;
+  if (!row_ok || !(isfinite(t0) && isfinite(P) && isfinite(a) && isfinite(inc) && isfinite(e) && isfinite(w)) ||
+      !(P > 0.0) || !(a > 0.0) || !(e >= 0.0 && e < 1.0)) {
+    c.flags = PV_BAD;
+    return;
+  }
+  c.t0 = t0; c.P = P; c.invP = 1.0 / P; c.a = a; c.e = e;
+  c.cosi = cos(inc);
+  const double k = c.khat;
+  const double margin = 1.0e-7;   // cycles; the cheap fold differs from the pinned one by < 2.3e-16 |x| <= 2.3e-8
+  double lo, hi;
+  if (e == 0.0) {
+    flags |= PV_CIRCULAR;
+    c.sinw = 0.0; c.cosw = 1.0; c.rt1me2 = 1.0; c.Mtr = 0.0;
+    // overlap needs a²(cos²i + sin²i sin²φ) < (1+k)² and cos φ > 0
+    const double ci2 = c.cosi * c.cosi;
+    const double si2 = 1.0 - ci2;
+    const double r = (1.0 + k) / a;
+    const double S = (r * r - ci2) / si2 + 1.0e-12;   // sin²φ below this value; si2 == 0 gives ±inf/NaN (handled)
+    if (S <= 0.0) { flags |= PV_NEVER; hi = 0.0; }
+    else if (!(S < 1.0)) hi = 0.25;
+    else hi = fmin(0.25, asin(sqrt(S)) * (1.0 / kTwoPi));
+    hi = hi * (1.0 + 1.0e-9) + margin;
+    lo = -hi;
+  } else {
+    sincos(w, &c.sinw, &c.cosw);
+    c.rt1me2 = sqrt((1.0 - e) * (1.0 + e));
+    const double ftr = 0.5 * kPi - w;
+    c.Mtr = mean_anomaly_of_true(ftr, e);
+    // overlap needs r |cos(w+f)| < 1+k and sin(w+f) > 0.  First bound with r >= a(1-e), then tighten with the smallest
+    // r on the resulting true-anomaly range (any in-transit f lies in the first range, so the second is still safe).
+    const double one_k = 1.0 + k;
+    double C = one_k / (a * (1.0 - e));
+    if (!(C < 1.0)) {
+      flags |= PV_ALWAYS; lo = -1.0; hi = 1.0;
+    } else {
+      double D = asin(C);
+      // max of cos f over [ftr-D, ftr+D]
+      const double fc = ftr - kTwoPi * rint(ftr * (1.0 / kTwoPi));   // reduce to [-π, π]
+      const double cmax = (fabs(fc) <= D) ? 1.0 : fmax(cos(fc - D), cos(fc + D));
+      const double rmin = a * (1.0 - e) * (1.0 + e) / fma(e, cmax, 1.0);
+      C = fmin(C, one_k / rmin);
+      D = asin(C) * (1.0 + 1.0e-9) + 1.0e-9;
+      double dhi = mean_anomaly_of_true(ftr + D, e) - c.Mtr;
+      double dlo = c.Mtr - mean_anomaly_of_true(ftr - D, e);
+      dhi -= kTwoPi * floor(dhi * (1.0 / kTwoPi));   // both differences are in [0, 2π)
+      dlo -= kTwoPi * floor(dlo * (1.0 / kTwoPi));
+      hi = dhi * (1.0 / kTwoPi) * (1.0 + 1.0e-9) + margin;
+      lo = -(dlo * (1.0 / kTwoPi) * (1.0 + 1.0e-9) + margin);
+      if (!(hi < 0.45 && lo > -0.45)) { flags |= PV_ALWAYS; lo = -1.0; hi = 1.0; }   // folded phase must not wrap
+    }
+  }
+  if (!(k > 0.0)) { flags |= PV_NEVER; }
+  c.ph_lo = lo; c.ph_hi = hi;
+  const double hx = (n_ss > 1) ? fabs(0.5 * t_exp * c.invP) * (1.0 + 1.0e-9) : 0.0;
+  c.ex_lo = lo - hx; c.ex_hi = hi + hx;
+  if (!(c.ex_hi < 0.49 && c.ex_lo > -0.49)) { flags |= PV_ALWAYS; }   // also catches a non-finite exposure width
+  c.flags = flags;
+}
+
+}  // namespace pt

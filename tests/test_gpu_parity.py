@@ -1,0 +1,303 @@
+"""Parity of the CUDA path (through the C ABI, via the thin binding) against the CPU oracle's __float128 instantiation
+on the same seeded inputs.  Gates (BASELINE.json north_star): exact fp64 flux 1e-12 abs; fp32 variant 2e-6 abs;
+interpolated path vs the oracle's interpolation of the SAME table 1e-12 abs."""
+import math
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from paper_1504_07433_b200 import inputs  # noqa: E402
+
+TOL64 = 1e-12
+TOL32 = 2e-6
+
+
+@pytest.fixture(scope="module")
+def pt():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_1504_07433_b200 as pkg
+    from paper_1504_07433_b200 import binding
+    assert binding.lib().pt_build_arch() == 100
+    return pkg
+
+
+def dev(x):
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def gpu_exact(pt, w, dtype=torch.float64, status=None):
+    f = pt.pt_ma_quad_exact(dev(w.times), dev(w.params), w.n_pb, w.n_ss, w.t_exp, dtype=dtype, status=status)
+    torch.cuda.synchronize()
+    return f.cpu().numpy()
+
+
+def ora_exact(oracle, w, prec="f128"):
+    return oracle.ma_quad_exact(w.times, w.params, w.n_pb, w.n_ss, w.t_exp, prec=prec)
+
+
+def oz64(oracle):
+    return lambda t, p: oracle.orbit_z(t, p, prec="f64")[:, :, 0]
+
+
+# ------------------------------------------------------------------------------------------- exact path, configs 1-3, 5
+def test_config1_full(pt, oracle, golden_config1):
+    w = inputs.config1()
+    f = gpu_exact(pt, w)
+    assert f.shape == (1, 1, 1000)
+    assert np.abs(f - ora_exact(oracle, w)).max() <= TOL64
+    # and straight against the stored worked example (values from the integral definitions)
+    w2 = inputs.Workload("g", golden_config1[:, 0].copy(), w.params)
+    assert np.abs(gpu_exact(pt, w2)[0, 0] - golden_config1[:, 2]).max() <= TOL64
+    z = pt.pt_orbit_z(dev(w2.times), dev(w2.params)).cpu().numpy()[0, :, 0]
+    assert np.abs(z - golden_config1[:, 1]).max() <= 1e-13
+
+
+@pytest.mark.parametrize("n_pv,n_t,n_ss", [(8, 5000, 10), (3, 1024, 10), (5, 1025, 3), (2, 2047, 1), (4, 700, 32),
+                                           (3, 333, 33), (2, 100, 70), (6, 1, 10), (2, 4097, 7)])
+def test_config2_reduced_supersampled(pt, oracle, n_pv, n_t, n_ss):
+    w = inputs.config2(n_pv=n_pv, n_t=n_t)
+    w.n_ss = n_ss
+    f = gpu_exact(pt, w)
+    r = ora_exact(oracle, w)
+    assert np.abs(f - r).max() <= TOL64
+    assert np.array_equal(f == 1.0, r == 1.0)   # out-of-transit samples are exactly 1 on both sides
+
+
+def test_config3_full_multipassband(pt, oracle):
+    w = inputs.config3()
+    f = gpu_exact(pt, w)
+    assert f.shape == (512, 20, 600)
+    assert np.abs(f - ora_exact(oracle, w)).max() <= TOL64
+
+
+@pytest.mark.parametrize("n_pb,n_t", [(1, 599), (3, 601), (20, 77), (64, 130)])
+def test_config3_ragged(pt, oracle, n_pb, n_t):
+    w = inputs.config3(n_pv=7, n_pb=n_pb, n_t=n_t)
+    assert np.abs(gpu_exact(pt, w) - ora_exact(oracle, w)).max() <= TOL64
+
+
+@pytest.mark.parametrize("order", ["sorted", "shuffled"])
+def test_config5_reduced(pt, oracle, order):
+    w = inputs.config5(oz64(oracle), n_pv=192, n_t=1100, order=order)
+    f = gpu_exact(pt, w)
+    r = ora_exact(oracle, w)
+    err = np.abs(f - r)
+    assert err.max() <= TOL64, (err.max(), np.unravel_index(np.argmax(err), err.shape))
+    z = pt.pt_orbit_z(dev(w.times), dev(w.params)).cpu().numpy()
+    zr = oracle.orbit_z(w.times, w.params, prec="f128")
+    assert np.abs(z - zr).max() <= 2e-13 * 20
+    assert np.array_equal(np.signbit(z), np.signbit(zr))
+
+
+def test_high_eccentricity_and_long_baseline(pt, oracle):
+    rng = np.random.default_rng(11)
+    n = 64
+    P = rng.uniform(1, 10, n)
+    e = np.concatenate([rng.uniform(0.6, 0.95, n // 2), rng.uniform(0.95, 0.99, n // 2)])
+    wv = rng.uniform(0, 2 * math.pi, n)
+    a = rng.uniform(8, 30, n)
+    b = rng.uniform(0, 0.9, n)
+    inc = np.arccos(np.clip(b * (1 + e * np.sin(wv)) / (a * (1 - e * e)), -1, 1))
+    params = np.stack([P * rng.uniform(0, 1, n), P, a, inc, e, wv, rng.uniform(0.02, 0.3, n), 0.4 + 0 * P, 0.2 + 0 * P], 1)
+    times = np.sort(rng.uniform(0, 3000, 6000))   # whole orbits, ~3000 d baseline (phase fold at |x| ~ 1e3)
+    w = inputs.Workload("ecc", times, params)
+    assert np.abs(gpu_exact(pt, w) - ora_exact(oracle, w)).max() <= TOL64
+    z = pt.pt_orbit_z(dev(times), dev(params)).cpu().numpy()
+    zr = oracle.orbit_z(times, params, prec="f128")
+    assert np.abs(z - zr).max() <= 1e-11
+
+
+# ------------------------------------------------------------------------------------------- degenerate inputs
+def test_edge_cases_k_and_geometry(pt, oracle):
+    t = np.linspace(-0.3, 0.3, 1501)
+    rows = []
+    for k in (0.0, 1e-8, 0.5, 0.999, 1.0, 1.5, 3.0):
+        for b in (0.0, 0.5, 1.0 + k, 1.0 + k + 1e-9):
+            a = 6.0
+            rows.append([0.0, 2.0, a, math.acos(min(1.0, b / a)), 0.0, 0.0, k, 0.3, 0.25])
+    rows.append([0.0, 2.0, 1.2, math.pi / 2, 0.0, 0.0, 0.4, 0.3, 0.25])    # a < 1+k: always overlapping on the near side
+    rows.append([0.0, 2.0, 6.0, 0.0, 0.0, 0.0, 0.1, 0.3, 0.25])            # face-on orbit, never transits
+    rows.append([0.0, 2.0, 1.5, 1.2, 0.5, 0.3, 0.2, 0.3, 0.25])            # a(1-e) < 1+k
+    rows.append([0.1, 2.0, 6.0, math.pi / 2, 0.0, 0.0, 0.1, 0.0, 0.0])     # uniform disk
+    w = inputs.Workload("edge", t, np.array(rows))
+    f, r = gpu_exact(pt, w), ora_exact(oracle, w)
+    assert np.abs(f - r).max() <= TOL64
+    # supersampled, exposure longer than the transit
+    w.n_ss, w.t_exp = 5, 0.2
+    assert np.abs(gpu_exact(pt, w) - ora_exact(oracle, w)).max() <= TOL64
+
+
+def test_exact_equality_special_cases_via_orbit(pt, oracle):
+    """b chosen so that z(t0) hits z = k, 1-k, 0 to within an ulp; plus the k = 1/2 neighbourhood."""
+    rows = []
+    a = 8.0
+    for k in (0.1, 0.3, 0.5, 0.5 + 1e-9, 0.5 - 1e-9, 0.7):
+        for zt in (k, abs(1 - k), 0.0, 1 + k, k * (1 + 1e-15), abs(1 - k) * (1 - 1e-15)):
+            rows.append([0.0, 3.0, a, math.acos(zt / a), 0.0, 0.0, k, 0.5, 0.1])
+    w = inputs.Workload("eq", np.array([0.0, 1e-9, -1e-9, 1e-6, 3.0, 1e-4]), np.array(rows))
+    assert np.abs(gpu_exact(pt, w) - ora_exact(oracle, w)).max() <= TOL64
+
+
+def test_bad_parameters_nan_rows_and_status(pt, oracle):
+    w = inputs.config2(n_pv=9, n_t=2100)
+    p = w.params
+    p[1, 1] = -1.0; p[2, 4] = 1.0; p[3, 6] = -0.1; p[4, 2] = np.nan; p[6, 7] = 3.0; p[6, 8] = 0.0   # last: 1 - u1/3 = 0
+    st = torch.zeros(2, dtype=torch.int32, device="cuda")
+    f = gpu_exact(pt, w, status=st)
+    r = ora_exact(oracle, w, "f64")
+    assert np.array_equal(np.isnan(f), np.isnan(r))
+    assert np.all(np.isnan(f[[1, 2, 3, 4, 6]])) and np.all(np.isfinite(f[[0, 5, 7, 8]]))
+    assert st.cpu().tolist() == [pt.PT_ST_BAD_PARAM, 5]
+    z = pt.pt_orbit_z(dev(w.times), dev(p)).cpu().numpy()
+    assert np.all(np.isnan(z[[1, 2, 3, 4, 6]])) and np.all(np.isfinite(z[0]))
+
+
+def test_argument_errors(pt):
+    from paper_1504_07433_b200 import binding
+    L = binding.lib()
+    t = torch.zeros(8, dtype=torch.float64, device="cuda")
+    p = torch.zeros((1, 9), dtype=torch.float64, device="cuda")
+    o = torch.zeros(8, dtype=torch.float64, device="cuda")
+    assert L.pt_ma_quad_exact(None, 8, 0, p.data_ptr(), 1, 1, 1, 0.0, 0, o.data_ptr(), None, None) == binding.PT_ERR_NULL
+    assert L.pt_ma_quad_exact(t.data_ptr(), 0, 0, p.data_ptr(), 1, 1, 1, 0.0, 0, o.data_ptr(), None, None) == binding.PT_ERR_SIZE
+    assert L.pt_ma_quad_exact(t.data_ptr(), 8, 0, p.data_ptr(), 1, 1, 0, 0.0, 0, o.data_ptr(), None, None) == binding.PT_ERR_SIZE
+    assert L.pt_ma_quad_exact(t.data_ptr(), 8, 4, p.data_ptr(), 1, 1, 1, 0.0, 0, o.data_ptr(), None, None) == binding.PT_ERR_SIZE
+    assert L.pt_ma_quad_exact(t.data_ptr(), 8, 0, p.data_ptr(), 1, 1, 1, 0.0, 7, o.data_ptr(), None, None) == binding.PT_ERR_DTYPE
+    assert L.pt_ma_table_build(0.1, 0.05, 4, 1.2, 4, 0, 3, o.data_ptr(), None) == binding.PT_ERR_SIZE
+    bad = binding.pt_table(None, 0, 4, 4, 3, 0.0, 0.1, 0.1)
+    import ctypes as C
+    assert L.pt_ma_quad_interp(C.byref(bad), t.data_ptr(), 8, 0, p.data_ptr(), 1, 1, 1, 0.0, 0, o.data_ptr(), None, None) == binding.PT_ERR_TABLE
+    with pytest.raises(binding.PtError):
+        pt.pt_ma_quad_exact(t.cpu(), p.cpu())
+
+
+def test_unaligned_output_and_odd_row_length(pt, oracle):
+    w = inputs.config2(n_pv=3, n_t=1501)
+    w.n_ss = 2
+    buf = torch.empty(3 * 1501 + 1, dtype=torch.float64, device="cuda")
+    out = buf[1:].view(3, 1, 1501)    # 8-byte aligned only
+    pt.pt_ma_quad_exact(dev(w.times), dev(w.params), 1, 2, w.t_exp, out=out)
+    assert np.abs(out.cpu().numpy() - ora_exact(oracle, w)).max() <= TOL64
+
+
+# ------------------------------------------------------------------------------------------- fp32 variant
+@pytest.mark.parametrize("cfg", ["c2", "c3", "c5"])
+def test_fp32_variant(pt, oracle, cfg):
+    w = {"c2": lambda: inputs.config2(n_pv=8, n_t=3000), "c3": lambda: inputs.config3(n_pv=32),
+         "c5": lambda: inputs.config5(oz64(oracle), n_pv=96, n_t=600)}[cfg]()
+    f = gpu_exact(pt, w, dtype=torch.float32)
+    assert f.dtype == np.float32
+    assert np.abs(f.astype(np.float64) - ora_exact(oracle, w)).max() <= TOL32
+
+
+# ------------------------------------------------------------------------------------------- table + interpolated path
+def _table_cfg(small=True):
+    return dict(k_min=0.05, k_max=0.25, n_k=41, z_max=1.25, n_z=1251) if small else inputs.config4(1, 1).table
+
+
+@pytest.mark.parametrize("dtype,n_fn", [(torch.float64, 3), (torch.float32, 4), (torch.float64, 4), (torch.float32, 3)])
+def test_table_build_parity(pt, oracle, dtype, n_fn):
+    c = _table_cfg()
+    tb = pt.pt_ma_table_build(dtype=dtype, n_fn=n_fn, **c)
+    torch.cuda.synchronize()
+    ref = oracle.ma_table_build(c["k_min"], c["k_max"], c["n_k"], c["z_max"], c["n_z"],
+                                np.float64 if dtype == torch.float64 else np.float32, n_fn, "f128")
+    got = tb.data.cpu().numpy()
+    tol = 1e-14 if dtype == torch.float64 else 6e-8
+    assert np.abs(got.astype(np.float64) - ref.astype(np.float64)).max() <= tol
+    dk, dz = oracle.table_spacing(c["k_min"], c["k_max"], c["n_k"], c["z_max"], c["n_z"])
+    assert tb.dk == dk and tb.dz == dz
+
+
+@pytest.mark.parametrize("tdtype,n_fn", [(torch.float64, 3), (torch.float32, 4)])
+def test_interp_vs_oracle_interp_of_same_table(pt, oracle, tdtype, n_fn):
+    c = _table_cfg()
+    tb = pt.pt_ma_table_build(dtype=tdtype, n_fn=n_fn, **c)
+    w = inputs.config4(n_pv=24, n_t=5003)
+    w.params[3, 6] = 0.3     # off the table: exact fallback + status bit
+    w.params[5, 6] = 0.25    # last node
+    w.params[6, 6] = 0.05    # first node
+    st = torch.zeros(2, dtype=torch.int32, device="cuda")
+    f = pt.pt_ma_quad_interp(tb, dev(w.times), dev(w.params), status=st).cpu().numpy()
+    host_tb = tb.data.cpu().numpy()      # the SAME table, downloaded
+    r = oracle.ma_quad_interp(host_tb, tb.k_min, tb.dk, tb.dz, w.times, w.params, prec="f128")
+    assert np.abs(f - r).max() <= TOL64
+    assert st.cpu().tolist() == [pt.PT_ST_K_OUT_OF_TABLE, 1]
+    # reported, not gated: error against the exact model
+    fe = ora_exact(oracle, w)
+    err = np.abs(f - fe)
+    print("interp vs exact: max %.3e mean(in transit) %.3e" % (err.max(), err[fe < 1].mean()))
+    assert err.max() < 5e-5
+    # supersampled + multi-passband through the table
+    w3 = inputs.config3(n_pv=5, n_pb=4, n_t=300)
+    w3.n_ss, w3.t_exp = 3, 0.002
+    f3 = pt.pt_ma_quad_interp(tb, dev(w3.times), dev(w3.params), 4, 3, w3.t_exp).cpu().numpy()
+    r3 = oracle.ma_quad_interp(host_tb, tb.k_min, tb.dk, tb.dz, w3.times, w3.params, 4, 3, w3.t_exp, prec="f128")
+    assert np.abs(f3 - r3).max() <= TOL64
+
+
+# ------------------------------------------------------------------------------------------- host-buffer entry points
+def test_host_entry_points(pt, oracle):
+    w = inputs.config2(n_pv=4, n_t=3000)
+    t, p = torch.from_numpy(w.times).pin_memory(), torch.from_numpy(w.params).pin_memory()
+    out = torch.empty((4, 1, 3000), dtype=torch.float64).pin_memory()
+    st = torch.zeros(2, dtype=torch.int32)
+    pt.pt_ma_quad_exact_host(t, p, out, 1, w.n_ss, w.t_exp, status=st)
+    assert np.abs(out.numpy() - ora_exact(oracle, w)).max() <= TOL64 and st.tolist() == [0, 0]
+    tb = pt.pt_ma_table_build(**_table_cfg())
+    w.n_ss = 1
+    pt.pt_ma_quad_interp_host(tb, t, p, out, 1, 1, 0.0)
+    r = oracle.ma_quad_interp(tb.data.cpu().numpy(), tb.k_min, tb.dk, tb.dz, w.times, w.params, prec="f128")
+    assert np.abs(out.numpy() - r).max() <= TOL64
+
+
+# ------------------------------------------------------------------------------------------- full sizes, sampled
+def test_config2_full_size_sampled(pt, oracle):
+    w = inputs.config2()
+    f = gpu_exact(pt, w)
+    assert f.shape == (64, 1, 60000)
+    rows = [0, 7, 21, 40, 63]
+    ws = inputs.Workload("s", w.times, w.params[rows], 1, w.n_ss, w.t_exp)
+    assert np.abs(f[rows] - ora_exact(oracle, ws)).max() <= TOL64
+    # properties that hold at any size: bounded, exactly 1 away from transit (checked through the product's own z)
+    assert f.max() == 1.0 and f.min() > 0.9
+    z = pt.pt_orbit_z(dev(w.times), dev(w.params), 1, w.n_ss, w.t_exp).cpu().numpy()
+    k = w.params[:, 6][:, None]
+    out = np.all((z < 0) | (z >= 1 + k[:, :, None]), axis=2)
+    assert np.all(f[:, 0][out] == 1.0) and np.all(f[:, 0][~out] < 1.0)
+
+
+def test_config4_full_size_sampled(pt, oracle):
+    w = inputs.config4()
+    c = w.table
+    res = {}
+    for tdtype in (torch.float32, torch.float64):
+        tb = pt.pt_ma_table_build(dtype=tdtype, n_fn=3, **c)
+        f = pt.pt_ma_quad_interp(tb, dev(w.times), dev(w.params))
+        torch.cuda.synchronize()
+        rows = [0, 1, 511, 2048, 4095]
+        host_rows = f[rows].cpu().numpy()
+        # oracle interpolation of the same table: download only the k-rows those parameter vectors touch
+        host_tb = tb.data.cpu().numpy()
+        ws = inputs.Workload("s", w.times, w.params[rows])
+        r = oracle.ma_quad_interp(host_tb, tb.k_min, tb.dk, tb.dz, ws.times, ws.params, prec="f128")
+        assert np.abs(host_rows - r).max() <= TOL64
+        fe = ora_exact(oracle, ws)
+        res[str(tdtype)] = (np.abs(host_rows - fe).max(), np.abs(host_rows - fe)[fe < 1].mean())
+        assert float(f.max()) == 1.0 and float(f.min()) > 0.9
+        del f, tb
+    print("config4 interp vs exact (max, mean in transit):", res)
+
+
+def test_config5_full_size_sampled(pt, oracle):
+    w = inputs.config5(oz64(oracle))
+    assert w.n_eval == 2 ** 24
+    f = gpu_exact(pt, w)
+    rows = np.arange(0, 4096, 61)
+    ws = inputs.Workload("s", w.times[rows], w.params[rows])
+    err = np.abs(f[rows] - ora_exact(oracle, ws))
+    assert err.max() <= TOL64, err.max()
+    assert f.max() <= 1.0 and f.min() >= 0.0
