@@ -21,7 +21,6 @@
 namespace pt {
 
 constexpr int kThreads = 256;
-constexpr int kTile = 1024;          // exposures per tile
 constexpr int kMaxPassbands = 1024;  // 3 doubles of shared memory each
 
 static std::atomic<int64_t> g_launches{0};
@@ -35,7 +34,8 @@ struct FluxArgs {
   double t_exp;
   void* flux;
   int32_t* status;
-  int tiles_per_pv, tiles_per_block, blocks_per_pv;
+  int blocks_per_pv;
+  int64_t exp_per_block;
   // interpolation table (mode 1)
   const void* tb;
   int tb_dtype, n_k, n_z, n_fn;
@@ -102,32 +102,49 @@ __device__ __forceinline__ Basis table_lookup(const FluxArgs& A, int ik, double 
   return b;
 }
 
+// Per-passband combine and streaming stores of one exposure's fluxes.
+template <typename OutT>
+__device__ __forceinline__ void store_exposure(OutT* __restrict__ out, int64_t n_t, int64_t e, int n_pb,
+                                               const double* __restrict__ coef, double le, double ld, double ed) {
+  for (int j = 0; j < n_pb; ++j) {
+    const double v = 1.0 - fma(coef[3 * j + 2], ed, fma(coef[3 * j + 1], ld, coef[3 * j] * le));
+    __stcs(out + (int64_t)j * n_t + e, (OutT)v);
+  }
+}
+template <typename OutT>
+__device__ __forceinline__ void store_ones(OutT* __restrict__ out, int64_t n_t, int64_t e, int n_pb) {
+  for (int j = 0; j < n_pb; ++j) __stcs(out + (int64_t)j * n_t + e, (OutT)1.0);
+}
+
 // MODE 0: exact.  MODE 1: interpolated (falls back to exact for a parameter vector whose k̂ is off the table).
+//
+// Every warp is autonomous after the per-block setup (no block barrier in the loop): it streams 32 exposures at a time,
+// stores flux = 1 for those that fail the window test, and keeps the others in a private 64-entry ring queue; as soon
+// as the queue holds a full batch (EPW = 32/G exposures, G = min(n_ss,32) lanes each) the warp evaluates it with all
+// lanes busy.  Warps of a block take interleaved 32-exposure groups, so in-transit work is spread over the block.
 template <int MODE, typename OutT>
 __global__ void __launch_bounds__(kThreads, 2) flux_kernel(const FluxArgs A) {
   extern __shared__ double s_coef[];   // 3 * n_pb
   __shared__ PvConst c;
-  __shared__ double s_le[kTile], s_ld[kTile], s_ed[kTile];
-  __shared__ unsigned short s_queue[kTile];
-  __shared__ int s_nq;
+  __shared__ uint32_t s_queue[kThreads / 32][64];
 
   const int64_t pv = blockIdx.x / A.blocks_per_pv;
   const int chunk = (int)(blockIdx.x % A.blocks_per_pv);
   const double* row = A.params + pv * (6 + 3 * (int64_t)A.n_pb);
-  const double* tt = A.times + pv * A.t_stride_pv;
-  OutT* out = (OutT*)A.flux + pv * A.n_pb * A.n_t;
+  const double* __restrict__ tt = A.times + pv * A.t_stride_pv;
+  OutT* __restrict__ out = (OutT*)A.flux + pv * A.n_pb * A.n_t;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int n_pb = A.n_pb;
 
-  block_setup(c, s_coef, row, A.n_pb, A.n_ss, A.t_exp);
+  block_setup(c, s_coef, row, n_pb, A.n_ss, A.t_exp);
 
-  const int tile_lo = chunk * A.tiles_per_block;
-  const int tile_hi = min(tile_lo + A.tiles_per_block, A.tiles_per_pv);
+  const int64_t e_begin = (int64_t)chunk * A.exp_per_block;
+  const int64_t e_end = min(e_begin + A.exp_per_block, A.n_t);
   const int flags = c.flags;
 
   if (flags & PV_BAD) {
-    const int64_t e_lo = (int64_t)tile_lo * kTile, e_hi = min((int64_t)tile_hi * kTile, A.n_t);
-    for (int j = 0; j < A.n_pb; ++j)
-      for (int64_t e = e_lo + tid; e < e_hi; e += kThreads) out[j * A.n_t + e] = (OutT)nan64();
+    for (int j = 0; j < n_pb; ++j)
+      for (int64_t e = e_begin + tid; e < e_end; e += kThreads) out[j * A.n_t + e] = (OutT)nan64();
     if (chunk == 0 && tid == 0 && A.status) {
       atomicOr(&A.status[0], PT_ST_BAD_PARAM);
       atomicAdd(&A.status[1], 1);
@@ -149,108 +166,77 @@ __global__ void __launch_bounds__(kThreads, 2) flux_kernel(const FluxArgs A) {
     }
   }
 
-  // lane -> (slot, g): G lanes per queued exposure, EPW exposures per warp pass
+  // lane -> (slot, g): G lanes per queued exposure, EPW exposures per batch
   const int n_ss = A.n_ss;
   const int G = n_ss < 32 ? n_ss : 32;
   const int EPW = 32 / G;
   const int slot = lane / G, g = lane - slot * G;
-  const bool lane_used = slot < EPW;
   const double off0 = (n_ss > 1) ? subsample_offset(g, n_ss, A.t_exp) : 0.0;
   const double inv_nss = 1.0 / (double)n_ss;
   const double khat = c.khat;
   const double ex_lo = c.ex_lo, ex_hi = c.ex_hi;
+  uint32_t* queue = s_queue[warp];
+  int qhead = 0, qcount = 0;   // warp-uniform
 
-  for (int tile = tile_lo; tile < tile_hi; ++tile) {
-    const int64_t e0 = (int64_t)tile * kTile;
-    const int n_e = (int)min((int64_t)kTile, A.n_t - e0);
-    if (tid == 0) s_nq = 0;
-    __syncthreads();
-
-    // ---- phase A: window test, queue build
-    if (!(flags & PV_NEVER)) {
-      for (int i = tid; i < kTile; i += kThreads) {
-        bool inw = false;
-        if (i < n_e) {
-          s_le[i] = 0.0; s_ld[i] = 0.0; s_ed[i] = 0.0;
-          inw = (flags & PV_ALWAYS) ? true : in_window(c, __ldg(tt + e0 + i), ex_lo, ex_hi);
-        }
-        const unsigned m = __ballot_sync(0xffffffffu, inw);
-        if (m) {
-          int base = 0;
-          if (lane == 0) base = atomicAdd(&s_nq, __popc(m));
-          base = __shfl_sync(0xffffffffu, base, 0);
-          if (inw) s_queue[base + __popc(m & ((1u << lane) - 1u))] = (unsigned short)i;
+  // evaluate the first `nb` queued exposures (nb <= EPW) with G lanes each
+  auto process_batch = [&](int nb) {
+    const bool act = slot < nb;
+    double ale = 0.0, ald = 0.0, aed = 0.0;
+    int64_t e = 0;
+    if (act) {
+      e = e_begin + queue[(qhead + slot) & 63];
+      const double t = __ldg(tt + e);
+      for (int s = g; s < n_ss; s += G) {
+        const double off = (s == g) ? off0 : subsample_offset(s, n_ss, A.t_exp);
+        const double ts = (n_ss > 1) ? __dadd_rn(t, off) : t;
+        const double ph = fold_phase(ts, c.t0, c.P);
+        const double zs = orbit_z_signed(c, ph);
+        if (zs >= 0.0 && zs < 1.0 + khat) {
+          Basis b;
+          if (MODE == 1 && use_table) {
+            b = (A.tb_dtype == PT_F64) ? table_lookup<double>(A, ik, fk, zs) : table_lookup<float>(A, ik, fk, zs);
+          } else {
+            b = ma_basis(khat, zs);
+          }
+          ale += b.le; ald += b.ld; aed += b.ed;
         }
       }
     }
-    __syncthreads();
-    const int nq = s_nq;
-
-    // ---- phase B: drain the queue with dense warps
-    for (int q0 = warp * EPW; q0 < nq; q0 += (kThreads / 32) * EPW) {
-      const int qi = q0 + slot;
-      const bool act = lane_used && qi < nq;
-      double ale = 0.0, ald = 0.0, aed = 0.0;
-      int el = 0;
-      if (act) {
-        el = s_queue[qi];
-        const double t = __ldg(tt + e0 + el);
-        for (int s = g; s < n_ss; s += G) {
-          const double off = (s == g) ? off0 : subsample_offset(s, n_ss, A.t_exp);
-          const double ts = (n_ss > 1) ? __dadd_rn(t, off) : t;
-          const double ph = fold_phase(ts, c.t0, c.P);
-          const double zs = orbit_z_signed(c, ph);
-          if (zs >= 0.0 && zs < 1.0 + khat) {
-            Basis b;
-            if (MODE == 1 && use_table) {
-              b = (A.tb_dtype == PT_F64) ? table_lookup<double>(A, ik, fk, zs) : table_lookup<float>(A, ik, fk, zs);
-            } else {
-              b = ma_basis(khat, zs);
-            }
-            ale += b.le; ald += b.ld; aed += b.ed;
-          }
-        }
-      }
-      if (G > 1) {   // segmented sum over the G lanes of each exposure (warp-uniform branch)
+    if (G > 1) {   // segmented sum over the G lanes of each exposure (warp-uniform branch, full-warp shuffles)
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-          const double tle = __shfl_down_sync(0xffffffffu, ale, o);
-          const double tld = __shfl_down_sync(0xffffffffu, ald, o);
-          const double ted = __shfl_down_sync(0xffffffffu, aed, o);
-          if (g + o < G) { ale += tle; ald += tld; aed += ted; }
-        }
-      }
-      if (act && g == 0) {
-        s_le[el] = ale * inv_nss; s_ld[el] = ald * inv_nss; s_ed[el] = aed * inv_nss;
+      for (int o = 1; o < 32; o <<= 1) {
+        const double tle = __shfl_down_sync(0xffffffffu, ale, o);
+        const double tld = __shfl_down_sync(0xffffffffu, ald, o);
+        const double ted = __shfl_down_sync(0xffffffffu, aed, o);
+        if (g + o < G) { ale += tle; ald += tld; aed += ted; }
       }
     }
-    __syncthreads();
+    if (act && g == 0) store_exposure(out, A.n_t, e, n_pb, s_coef, ale * inv_nss, ald * inv_nss, aed * inv_nss);
+    qhead = (qhead + nb) & 63;
+    qcount -= nb;
+  };
 
-    // ---- phase C: per-passband combine and coalesced stores
-    const bool all_one = (nq == 0);
-    // 16-byte stores: with n_t even every row start and tile start is 16-byte aligned if the base pointer is
-    const bool vec2 = (sizeof(OutT) == 8) && ((A.n_t & 1) == 0) && ((reinterpret_cast<uintptr_t>(A.flux) & 15) == 0);
-    for (int j = 0; j < A.n_pb; ++j) {
-      const double cA = s_coef[3 * j], cB = s_coef[3 * j + 1], cC = s_coef[3 * j + 2];
-      OutT* o = out + (int64_t)j * A.n_t + e0;
-      if (vec2) {
-        for (int i = 2 * tid; i < n_e; i += 2 * kThreads) {
-          double2 v;
-          if (all_one) { v.x = 1.0; v.y = 1.0; }
-          else {
-            v.x = 1.0 - fma(cC, s_ed[i], fma(cB, s_ld[i], cA * s_le[i]));
-            v.y = 1.0 - fma(cC, s_ed[i + 1], fma(cB, s_ld[i + 1], cA * s_le[i + 1]));
-          }
-          __stcs((double2*)(o + i), v);
-        }
-      } else {
-        for (int i = tid; i < n_e; i += kThreads) {
-          const double v = all_one ? 1.0 : 1.0 - fma(cC, s_ed[i], fma(cB, s_ld[i], cA * s_le[i]));
-          o[i] = (OutT)v;
-        }
-      }
+  const int64_t n_groups = (e_end - e_begin + 31) / 32;
+  const int64_t n_iter = (n_groups + kThreads / 32 - 1) / (kThreads / 32);   // same trip count for every warp
+  for (int64_t it = 0; it < n_iter; ++it) {
+    const int64_t e = e_begin + (it * (kThreads / 32) + warp) * 32 + lane;
+    const bool valid = e < e_end;
+    bool inw = false;
+    if (valid) {
+      if (flags & PV_NEVER) inw = false;
+      else if (flags & PV_ALWAYS) inw = true;
+      else inw = in_window(c, __ldg(tt + e), ex_lo, ex_hi);
+      if (!inw) store_ones(out, A.n_t, e, n_pb);
     }
-    __syncthreads();
+    const unsigned m = __ballot_sync(0xffffffffu, inw);
+    if (inw) queue[(qhead + qcount + __popc(m & ((1u << lane) - 1u))) & 63] = (uint32_t)(e - e_begin);
+    qcount += __popc(m);
+    __syncwarp();
+    const bool last = (it + 1 == n_iter);
+    while (qcount >= EPW || (last && qcount > 0)) {   // full batches; the ragged remainder only after the last group
+      process_batch(min(qcount, EPW));
+    }
+    __syncwarp();
   }
 }
 
@@ -348,16 +334,17 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
     A.tb = tb->d_data; A.tb_dtype = tb->dtype; A.n_k = tb->n_k; A.n_z = tb->n_z; A.n_fn = tb->n_fn;
     A.k_min = tb->k_min; A.dk = tb->dk; A.dz = tb->dz; A.inv_dk = 1.0 / tb->dk; A.inv_dz = 1.0 / tb->dz;
   }
-  const int64_t tiles_per_pv = (n_t + kTile - 1) / kTile;
-  if (tiles_per_pv > 0x7fffffff) return PT_ERR_SIZE;
+  // exposures per block: a multiple of 256 (32 per warp-iteration), at least 2048 when the row is that long, chosen so
+  // that the grid has about 8 blocks per SM
   const int64_t target_blocks = 148 * 8;
   int64_t bpp = (target_blocks + n_pv - 1) / n_pv;
-  if (bpp > tiles_per_pv) bpp = tiles_per_pv;
-  if (bpp < 1) bpp = 1;
-  const int64_t tpb = (tiles_per_pv + bpp - 1) / bpp;
-  bpp = (tiles_per_pv + tpb - 1) / tpb;
+  int64_t epb = (n_t + bpp - 1) / bpp;
+  if (epb < 2048) epb = 2048;
+  epb = (epb + 255) / 256 * 256;
+  if (epb > ((int64_t)1 << 31)) return PT_ERR_SIZE;
+  bpp = (n_t + epb - 1) / epb;
   if (n_pv * bpp > 0x7fffffff) return PT_ERR_SIZE;
-  A.tiles_per_pv = (int)tiles_per_pv; A.tiles_per_block = (int)tpb; A.blocks_per_pv = (int)bpp;
+  A.blocks_per_pv = (int)bpp; A.exp_per_block = epb;
   const dim3 grid((unsigned)(n_pv * bpp));
   const size_t smem = (size_t)3 * n_pb * sizeof(double);
   if (mode == 0) {
