@@ -223,7 +223,8 @@ def run_ours(args):
     clocks = sampler.result()
 
     extra = {}
-    if rank == 0 and not args.headline_only:
+    sections = set(args.sections.split(","))
+    if rank == 0 and "scaled" in sections:
         # -------------------------------------------------------------- scaled configs[1] (448 pv, 2.7e8 evals)
         ws = inputs.config2(n_pv=448)
         st, sp = to_dev(ws.times), to_dev(ws.params)
@@ -235,6 +236,7 @@ def run_ours(args):
                            "ms": t_s * 1e3, "in_transit_frac": n_in_s / ws.n_eval,
                            "fp64_frac_of_model_peak": alg_s / t_s / fp64_model_peak}
         del st, sp, so
+    if rank == 0 and "dense" in sections:
         # -------------------------------------------------------------- dense: every sample in transit, eccentric
         wd = inputs.dense_transit(n_pv=4096, n_t=4096)
         dt_, dp_ = to_dev(wd.times), to_dev(wd.params)
@@ -251,6 +253,7 @@ def run_ours(args):
         t_d32 = _time_steps(lambda: pt.pt_ma_quad_exact(dt_, dp_, dtype=torch.float32, out=do32), 10, 3, flush, 1) / 10
         extra["dense"]["fp32_variant_value"] = wd.n_eval / t_d32
         del dt_, dp_, do, do32
+    if rank == 0 and "interp" in sections:
         # -------------------------------------------------------------- configs[3]: table build + interpolated path
         wi = inputs.config4()
         c = wi.table
@@ -271,6 +274,7 @@ def run_ours(args):
         res_i["workload"] = "BASELINE.json configs[3]: 4096 pv x 100000 times, table 401 x 12501, fp64 flux (3.28 GB/launch > L2)"
         extra["interp"] = res_i
         del it_, ip_, io
+    if rank == 0 and "cpu" in sections:
         # -------------------------------------------------------------- CPU baseline: the oracle as it stands
         from oracle import pt_oracle
         pt_oracle.build()
@@ -340,7 +344,8 @@ def main():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--headline-only", action="store_true", help="skip the scaled/dense/interp/cpu_baseline extras")
+    ap.add_argument("--sections", default="scaled,dense,interp,cpu",
+                    help="extra sections to run besides the headline: any of scaled,dense,interp,cpu (or 'none')")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

@@ -22,6 +22,8 @@ namespace pt {
 
 constexpr int kThreads = 256;
 constexpr int kMaxPassbands = 1024;  // 3 doubles of shared memory each
+constexpr int kUnroll = 4;            // 32-exposure groups a warp streams per iteration (independent loads in flight)
+constexpr int kQueue = 512;           // per-warp ring queue: > 2*32*kUnroll + 32 entries, power of two
 
 static std::atomic<int64_t> g_launches{0};
 
@@ -103,48 +105,66 @@ __device__ __forceinline__ Basis table_lookup(const FluxArgs& A, int ik, double 
 }
 
 // Per-passband combine and streaming stores of one exposure's fluxes.
-template <typename OutT>
-__device__ __forceinline__ void store_exposure(OutT* __restrict__ out, int64_t n_t, int64_t e, int n_pb,
+template <bool NPB1, typename OutT>
+__device__ __forceinline__ void store_exposure(OutT* __restrict__ out, int64_t n_t, int n_pb,
                                                const double* __restrict__ coef, double le, double ld, double ed) {
-  for (int j = 0; j < n_pb; ++j) {
-    const double v = 1.0 - fma(coef[3 * j + 2], ed, fma(coef[3 * j + 1], ld, coef[3 * j] * le));
-    __stcs(out + (int64_t)j * n_t + e, (OutT)v);
+  if (NPB1) {
+    __stcs(out, (OutT)(1.0 - fma(coef[2], ed, fma(coef[1], ld, coef[0] * le))));
+  } else {
+    for (int j = 0; j < n_pb; ++j) {
+      const double v = 1.0 - fma(coef[3 * j + 2], ed, fma(coef[3 * j + 1], ld, coef[3 * j] * le));
+      __stcs(out + (int64_t)j * n_t, (OutT)v);
+    }
   }
 }
-template <typename OutT>
-__device__ __forceinline__ void store_ones(OutT* __restrict__ out, int64_t n_t, int64_t e, int n_pb) {
-  for (int j = 0; j < n_pb; ++j) __stcs(out + (int64_t)j * n_t + e, (OutT)1.0);
+template <bool NPB1, typename OutT>
+__device__ __forceinline__ void store_one(OutT* __restrict__ out, int64_t n_t, int n_pb) {
+  if (NPB1) __stcs(out, (OutT)1.0);
+  else for (int j = 0; j < n_pb; ++j) __stcs(out + (int64_t)j * n_t, (OutT)1.0);
+}
+template <typename OutT> struct Vec2;
+template <> struct Vec2<double> { typedef double2 type; };
+template <> struct Vec2<float> { typedef float2 type; };
+template <bool NPB1, typename OutT>
+__device__ __forceinline__ void store_one_pair(OutT* __restrict__ out, int64_t n_t, int n_pb) {
+  typename Vec2<OutT>::type v;
+  v.x = (OutT)1.0; v.y = (OutT)1.0;
+  if (NPB1) __stcs((typename Vec2<OutT>::type*)out, v);
+  else for (int j = 0; j < n_pb; ++j) __stcs((typename Vec2<OutT>::type*)(out + (int64_t)j * n_t), v);
 }
 
 // MODE 0: exact.  MODE 1: interpolated (falls back to exact for a parameter vector whose k̂ is off the table).
+// V: exposures per lane and load/store (2 = 16-byte ld/st.v2.f64, needs even row lengths and 16-byte aligned bases).
+// NPB1: single passband (one store per exposure, no passband loop).
 //
-// Every warp is autonomous after the per-block setup (no block barrier in the loop): it streams 32 exposures at a time,
-// stores flux = 1 for those that fail the window test, and keeps the others in a private 64-entry ring queue; as soon
-// as the queue holds a full batch (EPW = 32/G exposures, G = min(n_ss,32) lanes each) the warp evaluates it with all
-// lanes busy.  Warps of a block take interleaved 32-exposure groups, so in-transit work is spread over the block.
-template <int MODE, typename OutT>
+// Every warp is autonomous after the per-block setup (no block barrier in the loop): it streams kUnroll*32*V exposures
+// at a time (all loads issued first), stores flux = 1 for those that fail the phase-window test, and keeps the others in
+// a private ring queue; as soon as the queue holds a full batch (EPW = 32/G exposures, G = min(n_ss,32) lanes each) the
+// warp evaluates it with all lanes busy.  Warps of a block take interleaved super-groups, so in-transit work is spread
+// over the block.
+template <int MODE, int V, bool NPB1, typename OutT>
 __global__ void __launch_bounds__(kThreads, 2) flux_kernel(const FluxArgs A) {
   extern __shared__ double s_coef[];   // 3 * n_pb
   __shared__ PvConst c;
-  __shared__ uint32_t s_queue[kThreads / 32][64];
+  __shared__ uint32_t s_queue[kThreads / 32][kQueue];
 
   const int64_t pv = blockIdx.x / A.blocks_per_pv;
   const int chunk = (int)(blockIdx.x % A.blocks_per_pv);
   const double* row = A.params + pv * (6 + 3 * (int64_t)A.n_pb);
-  const double* __restrict__ tt = A.times + pv * A.t_stride_pv;
-  OutT* __restrict__ out = (OutT*)A.flux + pv * A.n_pb * A.n_t;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int n_pb = A.n_pb;
+  const int n_pb = NPB1 ? 1 : A.n_pb;
 
   block_setup(c, s_coef, row, n_pb, A.n_ss, A.t_exp);
 
   const int64_t e_begin = (int64_t)chunk * A.exp_per_block;
-  const int64_t e_end = min(e_begin + A.exp_per_block, A.n_t);
+  const uint32_t n_e = (uint32_t)min((int64_t)A.exp_per_block, A.n_t - e_begin);   // exposures of this block (< 2^31)
+  const double* __restrict__ tb = A.times + pv * A.t_stride_pv + e_begin;
+  OutT* __restrict__ ob = (OutT*)A.flux + pv * n_pb * A.n_t + e_begin;
   const int flags = c.flags;
 
   if (flags & PV_BAD) {
     for (int j = 0; j < n_pb; ++j)
-      for (int64_t e = e_begin + tid; e < e_end; e += kThreads) out[j * A.n_t + e] = (OutT)nan64();
+      for (uint32_t e = tid; e < n_e; e += kThreads) ob[(int64_t)j * A.n_t + e] = (OutT)nan64();
     if (chunk == 0 && tid == 0 && A.status) {
       atomicOr(&A.status[0], PT_ST_BAD_PARAM);
       atomicAdd(&A.status[1], 1);
@@ -174,7 +194,7 @@ __global__ void __launch_bounds__(kThreads, 2) flux_kernel(const FluxArgs A) {
   const double off0 = (n_ss > 1) ? subsample_offset(g, n_ss, A.t_exp) : 0.0;
   const double inv_nss = 1.0 / (double)n_ss;
   const double khat = c.khat;
-  const double ex_lo = c.ex_lo, ex_hi = c.ex_hi;
+  const double w_t0 = c.t0, w_invP = c.invP, w_mid = c.win_mid, w_half = c.win_half;
   uint32_t* queue = s_queue[warp];
   int qhead = 0, qcount = 0;   // warp-uniform
 
@@ -182,10 +202,10 @@ __global__ void __launch_bounds__(kThreads, 2) flux_kernel(const FluxArgs A) {
   auto process_batch = [&](int nb) {
     const bool act = slot < nb;
     double ale = 0.0, ald = 0.0, aed = 0.0;
-    int64_t e = 0;
+    uint32_t e = 0;
     if (act) {
-      e = e_begin + queue[(qhead + slot) & 63];
-      const double t = __ldg(tt + e);
+      e = queue[(qhead + slot) & (kQueue - 1)];
+      const double t = __ldg(tb + e);
       for (int s = g; s < n_ss; s += G) {
         const double off = (s == g) ? off0 : subsample_offset(s, n_ss, A.t_exp);
         const double ts = (n_ss > 1) ? __dadd_rn(t, off) : t;
@@ -211,32 +231,72 @@ __global__ void __launch_bounds__(kThreads, 2) flux_kernel(const FluxArgs A) {
         if (g + o < G) { ale += tle; ald += tld; aed += ted; }
       }
     }
-    if (act && g == 0) store_exposure(out, A.n_t, e, n_pb, s_coef, ale * inv_nss, ald * inv_nss, aed * inv_nss);
-    qhead = (qhead + nb) & 63;
+    if (act && g == 0)
+      store_exposure<NPB1>(ob + e, A.n_t, n_pb, s_coef, ale * inv_nss, ald * inv_nss, aed * inv_nss);
+    qhead = (qhead + nb) & (kQueue - 1);
     qcount -= nb;
   };
 
-  const int64_t n_groups = (e_end - e_begin + 31) / 32;
-  const int64_t n_iter = (n_groups + kThreads / 32 - 1) / (kThreads / 32);   // same trip count for every warp
-  for (int64_t it = 0; it < n_iter; ++it) {
-    const int64_t e = e_begin + (it * (kThreads / 32) + warp) * 32 + lane;
-    const bool valid = e < e_end;
-    bool inw = false;
-    if (valid) {
-      if (flags & PV_NEVER) inw = false;
-      else if (flags & PV_ALWAYS) inw = true;
-      else inw = in_window(c, __ldg(tt + e), ex_lo, ex_hi);
-      if (!inw) store_ones(out, A.n_t, e, n_pb);
+  // super-groups of kUnroll x 32 lanes x V exposures, interleaved over the warps of the block
+  constexpr int kWarps = kThreads / 32;
+  constexpr uint32_t kSuper = 32u * kUnroll * V;
+  const uint32_t n_super = (n_e + kSuper - 1) / kSuper;
+  const uint32_t n_iter = (n_super + kWarps - 1) / kWarps;   // same trip count for every warp
+  for (uint32_t it = 0; it < n_iter; ++it) {
+    const uint32_t base = (it * kWarps + warp) * kSuper;      // may lie beyond n_e for the last iteration
+    const bool full = base + kSuper <= n_e;                    // warp-uniform
+    double t[kUnroll][V];
+    unsigned inw = 0;                                          // bit (u*V+v): exposure (u,v) of this lane is in the window
+    if (full) {
+#pragma unroll
+      for (int u = 0; u < kUnroll; ++u) {                      // all loads first: kUnroll independent requests per lane
+        const uint32_t e = base + (u * 32 + lane) * V;
+        if (V == 2) { const double2 tv = __ldg((const double2*)(tb + e)); t[u][0] = tv.x; t[u][V - 1] = tv.y; }
+        else t[u][0] = __ldg(tb + e);
+      }
+#pragma unroll
+      for (int u = 0; u < kUnroll; ++u) {
+        const uint32_t e = base + (u * 32 + lane) * V;
+#pragma unroll
+        for (int v = 0; v < V; ++v) inw |= in_window(t[u][v], w_t0, w_invP, w_mid, w_half) ? (1u << (u * V + v)) : 0u;
+        const unsigned pair = (inw >> (u * V)) & (V == 2 ? 3u : 1u);
+        if (V == 2 && pair == 0) store_one_pair<NPB1>(ob + e, A.n_t, n_pb);
+        else {
+#pragma unroll
+          for (int v = 0; v < V; ++v) if (!((pair >> v) & 1u)) store_one<NPB1>(ob + e + v, A.n_t, n_pb);
+        }
+      }
+    } else {
+#pragma unroll
+      for (int u = 0; u < kUnroll; ++u) {
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+          const uint32_t e = base + (u * 32 + lane) * V + v;
+          if (e < n_e) {
+            if (in_window(__ldg(tb + e), w_t0, w_invP, w_mid, w_half)) inw |= 1u << (u * V + v);
+            else store_one<NPB1>(ob + e, A.n_t, n_pb);
+          }
+        }
+      }
     }
-    const unsigned m = __ballot_sync(0xffffffffu, inw);
-    if (inw) queue[(qhead + qcount + __popc(m & ((1u << lane) - 1u))) & 63] = (uint32_t)(e - e_begin);
-    qcount += __popc(m);
-    __syncwarp();
+    if (__any_sync(0xffffffffu, inw != 0)) {
+#pragma unroll
+      for (int uv = 0; uv < kUnroll * V; ++uv) {
+        const bool b = (inw >> uv) & 1u;
+        const unsigned m = __ballot_sync(0xffffffffu, b);
+        if (b) queue[(qhead + qcount + __popc(m & ((1u << lane) - 1u))) & (kQueue - 1)] =
+            base + ((uv / V) * 32 + lane) * V + (uv % V);
+        qcount += __popc(m);
+      }
+      __syncwarp();
+    }
     const bool last = (it + 1 == n_iter);
-    while (qcount >= EPW || (last && qcount > 0)) {   // full batches; the ragged remainder only after the last group
-      process_batch(min(qcount, EPW));
+    if (qcount >= EPW || (last && qcount > 0)) {
+      do {   // full batches; the ragged remainder only after the last group
+        process_batch(min(qcount, EPW));
+      } while (qcount >= EPW || (last && qcount > 0));
+      __syncwarp();
     }
-    __syncwarp();
   }
 }
 
@@ -347,13 +407,25 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   A.blocks_per_pv = (int)bpp; A.exp_per_block = epb;
   const dim3 grid((unsigned)(n_pv * bpp));
   const size_t smem = (size_t)3 * n_pb * sizeof(double);
+  // 16-byte loads/stores need even row lengths/strides and 16-byte aligned bases
+  const bool v2 = (n_t % 2 == 0) && (t_stride_pv % 2 == 0) && (reinterpret_cast<uintptr_t>(d_times) % 16 == 0) &&
+                  (reinterpret_cast<uintptr_t>(d_flux) % 16 == 0);
+  const bool p1 = (n_pb == 1);
+#define PT_LAUNCH(M, VV, P, T) flux_kernel<M, VV, P, T><<<grid, kThreads, smem, st>>>(A)
+#define PT_LAUNCH_T(M, T)                                    \
+  do {                                                       \
+    if (v2 && p1) PT_LAUNCH(M, 2, true, T);                  \
+    else if (v2) PT_LAUNCH(M, 2, false, T);                  \
+    else if (p1) PT_LAUNCH(M, 1, true, T);                   \
+    else PT_LAUNCH(M, 1, false, T);                          \
+  } while (0)
   if (mode == 0) {
-    if (dtype == PT_F64) flux_kernel<0, double><<<grid, kThreads, smem, st>>>(A);
-    else flux_kernel<0, float><<<grid, kThreads, smem, st>>>(A);
+    if (dtype == PT_F64) PT_LAUNCH_T(0, double); else PT_LAUNCH_T(0, float);
   } else {
-    if (dtype == PT_F64) flux_kernel<1, double><<<grid, kThreads, smem, st>>>(A);
-    else flux_kernel<1, float><<<grid, kThreads, smem, st>>>(A);
+    if (dtype == PT_F64) PT_LAUNCH_T(1, double); else PT_LAUNCH_T(1, float);
   }
+#undef PT_LAUNCH_T
+#undef PT_LAUNCH
   g_launches.fetch_add(1);
   return cudaGetLastError() == cudaSuccess ? PT_OK : PT_ERR_CUDA;
 }

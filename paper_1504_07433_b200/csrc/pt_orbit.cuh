@@ -21,6 +21,7 @@ struct PvConst {
   double khat;
   double ph_lo, ph_hi;   // conservative phase window of the transit (cycles, relative to conjunction), sample-level
   double ex_lo, ex_hi;   // the same widened by half an exposure: exposure-level test on the exposure centre
+  double win_mid, win_half;   // centre / half-width of [ex_lo, ex_hi]; half = -inf: never in transit, +inf: always
   int flags;
 };
 
@@ -35,12 +36,18 @@ __device__ __forceinline__ double subsample_offset(int s, int n_ss, double t_exp
   return __dmul_rn(t_exp, __dsub_rn(__ddiv_rn((double)s + 0.5, (double)n_ss), 0.5));
 }
 
-// Cheap window test on a time: is the sample possibly in transit?  Uses t*invP (not the pinned fold) and is only ever
-// used to SKIP samples whose flux is exactly 1; the window carries a margin far above the difference between the folds.
-__device__ __forceinline__ bool in_window(const PvConst& c, double t, double lo, double hi) {
-  const double x = (t - c.t0) * c.invP;
-  const double ph = x - rint(x);
-  return ((ph > lo) & (ph < hi)) | (fabs(x) > 1.0e8);
+// Cheap window test on an exposure time: can any subsample of it be in transit?  It is only ever used to SKIP exposures
+// whose flux is exactly 1, so it must never say "no" wrongly: it folds with (t-t0)*(1/P) instead of the pinned division
+// and rounds with the 1.5*2^52 trick, both of which differ from the pinned fold by less than 1e-15 |x| cycles — the
+// window is widened by exactly that (plus the fixed 1e-7 margin built into mid/half).  For |x| >= 2^51 the widened
+// half-width exceeds 2, so the test passes whatever the rounding did; NaN/inf times fail it (flux 1, as in the oracle,
+// where every comparison with NaN is false).  6 FP64-pipe instructions per exposure.
+__device__ __forceinline__ bool in_window(double t, double t0, double invP, double mid, double half) {
+  const double x = (t - t0) * invP;
+  const double magic = 6755399441055744.0;   // 1.5 * 2^52
+  const double r = __dsub_rn(__dadd_rn(x, magic), magic);
+  const double ph = x - r;
+  return fabs(ph - mid) < fma(fabs(x), 1.0e-15, half);
 }
 
 // Eccentric anomaly from mean anomaly M in (-π, π] by Newton's method.  Starter: for e <= 0.8 the third-order
@@ -165,6 +172,10 @@ __device__ inline void pv_setup_orbit(PvConst& c, const double* row, bool row_ok
   const double hx = (n_ss > 1) ? fabs(0.5 * t_exp * c.invP) * (1.0 + 1.0e-9) : 0.0;
   c.ex_lo = lo - hx; c.ex_hi = hi + hx;
   if (!(c.ex_hi < 0.49 && c.ex_lo > -0.49)) { flags |= PV_ALWAYS; }   // also catches a non-finite exposure width
+  c.win_mid = 0.5 * (c.ex_lo + c.ex_hi);
+  c.win_half = 0.5 * (c.ex_hi - c.ex_lo);
+  if (flags & PV_ALWAYS) { c.win_mid = 0.0; c.win_half = CUDART_INF; }
+  if (flags & PV_NEVER) { c.win_mid = 0.0; c.win_half = -CUDART_INF; }
   c.flags = flags;
 }
 
