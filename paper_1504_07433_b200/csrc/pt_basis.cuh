@@ -9,6 +9,8 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include "pt_math.cuh"
+
 namespace pt {
 
 struct Basis {
@@ -19,21 +21,21 @@ constexpr double kPi = 3.14159265358979323846;
 constexpr double kInvPi = 0.31830988618379067154;
 constexpr double kTwoThirds = 0.66666666666666666667;
 
-// cK·K(m) + cE·E(m) + cP·cel(kc, 1-n, a2, b2n) with mc = 1-m = kc² and sp = sqrt(1-n) > 0 the square root of the second
-// sequence's p-argument.  (a2, b2n) = (1, 1) makes the second integral Π(n|m); (0, n) makes it Π(n|m) - K(m).
-__device__ __forceinline__ double cel_pair(double mc, double sp, double cK, double cE, double cP, double a2, double b2n) {
-  double qc = sqrt(mc);
+// cK·K(m) + cE·E(m) + cP·cel(kc, 1-n, a2, b2·sp) with mc = 1-m = kc² and sp = sqrt(1-n) > 0 the square root of the second
+// sequence's p-argument.  (a2, b2) = (1, 1/sp) makes the second integral Π(n|m); (0, n/sp) makes it Π(n|m) - K(m).
+__device__ __forceinline__ double cel_pair(double mc, double sp, double cK, double cE, double cP, double a2, double b2) {
+  double qc = sqrt_fast(mc);
   // sequence 1 (p = 1): its p-iterate equals the ladder's `em`, and e/p equals the previous qc, so it needs 1/em only
   double a1 = cK + cE;
   double b1 = fma(cE, mc, cK);
-  // sequence 2: p2 = sqrt(1-n), b = b/p2
+  // sequence 2: p2 = sqrt(1-n); b2 arrives already divided by p2
   double p2 = sp;
-  double b2 = b2n / sp;
   double e = qc, em = 1.0;
 #pragma unroll 1
   for (int it = 0; it < 16; ++it) {
-    const double rem = 1.0 / em;
-    const double rp2 = 1.0 / p2;
+    const double rr = rcp_fast(em * p2);   // one reciprocal serves both sequences
+    const double rem = rr * p2;
+    const double rp2 = rr * em;
     // sequence 1
     double f = a1;
     a1 = fma(b1, rem, a1);
@@ -50,18 +52,20 @@ __device__ __forceinline__ double cel_pair(double mc, double sp, double cK, doub
     const double g = em;
     em += qc;
     if (fabs(g - qc) <= 1.0e-8 * g) break;
-    qc = sqrt(e);
-    qc += qc;
+    qc = 2.0 * sqrt_fast(e);
     e = qc * em;
   }
-  const double s1 = fma(a1, em, b1) / (2.0 * em * em);
-  const double s2 = fma(a2, em, b2) / (em * (em + p2));
+  const double d1 = 2.0 * em * em, d2 = em * (em + p2);
+  const double rr = rcp_fast(d1 * d2);
+  const double s1 = fma(a1, em, b1) * (d2 * rr);
+  const double s2 = fma(a2, em, b2) * (d1 * rr);
   return (0.5 * kPi) * fma(cP, s2, s1);
 }
 
 // Basis functions at radius ratio p > 0 and separation z >= 0 (planet in front of the star).
 __device__ __forceinline__ Basis ma_basis(double p, double z) {
   Basis r;
+  z = fmax(z, 1.0e-150);   // keeps every operand of the fast reciprocals normal; changes nothing above 1e-150
   // d = z-p, s = z+p and the four contact distances 1-d, 1+d, s-1, s+1.  Each is formed so that the operand pair that
   // nearly cancels at "its" contact is subtracted exactly first (Sterbenz), e.g. s-1 = z + (p-1) for p in [1/2, 2]:
   // a plain (z+p)-1 loses z entirely when z << p ~ 1 (and mc = (s-1)(s+1)/(4zp) then has O(1) relative error).
@@ -80,7 +84,7 @@ __device__ __forceinline__ Basis ma_basis(double p, double z) {
   const bool partial = sm1 > 0.0;
 
   if (partial) {
-    const double T = sqrt(oma * sm1 * sp1);
+    const double T = sqrt_fast(oma * sm1 * sp1);
     const double pp1 = pm1 * (p + 1.0);                  // p² - 1 without cancellation for p ~ 1
     const double kap0 = atan2(T, z2 + pp1);
     const double kap1 = atan2(T, z2 - pp1);
@@ -92,30 +96,32 @@ __device__ __forceinline__ Basis ma_basis(double p, double z) {
   }
 
   if (sm1 == 0.0) {  // inner contact z = 1-p: elementary closed form (exact equality only; table nodes land here)
-    r.ld = (2.0 / 3.0 * kInvPi) * acos(1.0 - 2.0 * p) - (4.0 / 9.0 * kInvPi) * (3.0 + 2.0 * p - 8.0 * p2) * sqrt(p * (1.0 - p));
+    r.ld = (2.0 / 3.0 * kInvPi) * acos(1.0 - 2.0 * p) - (4.0 / 9.0 * kInvPi) * (3.0 + 2.0 * p - 8.0 * p2) * sqrt(p * (1.0 - p));  // rare branch: library sqrt/acos are fine here
     return r;
   }
 
   double mc, sp, cK, cE, cP, pref, add;
-  double a2 = 1.0, b2n = 1.0;
+  double a2 = 1.0, b2;
   if (fabs(d) < 1.0e-100) {  // z = p: the Π term drops out
     add = 1.0 / 3.0;
     cP = 0.0;
     sp = 1.0;
+    b2 = 1.0;
     if (!partial) {  // p < 1/2, m = 4p²
       mc = (1.0 - 2.0 * p) * (1.0 + 2.0 * p);
       cE = 4.0 * (2.0 * p2 - 1.0);
       cK = mc;
       pref = 2.0 / 9.0 * kInvPi;
     } else {  // p > 1/2, m = 1/(4p²)
-      const double i4p2 = 1.0 / (4.0 * p2);
+      const double i4p2 = rcp_fast(4.0 * p2);
       mc = (2.0 * p - 1.0) * (2.0 * p + 1.0) * i4p2;
       cE = 16.0 * p * (2.0 * p2 - 1.0);
-      cK = -(1.0 - 4.0 * p2) * (3.0 - 8.0 * p2) / p;
+      cK = -(1.0 - 4.0 * p2) * (3.0 - 8.0 * p2) * rcp_fast(p);
       pref = 1.0 / 9.0 * kInvPi;
     }
   } else {
-    const double rd = 1.0 / d;
+    const double rd = rcp_fast(d);
+    const double ad = fabs(d);
     const double q = -d * s;  // p² - z²
     const double w7 = z2 + 7.0 * p2 - 4.0;
     add = d < 0.0 ? kTwoThirds : 0.0;
@@ -123,10 +129,12 @@ __device__ __forceinline__ Basis ma_basis(double p, double z) {
     if (partial) {
       const double a = d * d, b = s * s;
       const double pz = p * z;
-      mc = sm1 * sp1 / (4.0 * pz);
+      const double rpz = rsqrt_fast(pz);
+      mc = 0.25 * sm1 * sp1 * (rpz * rpz);
       sp = fabs(rd);          // sqrt(1/a)
+      b2 = ad;                // 1/sp
       cE = 4.0 * pz * w7;
-      pref = (1.0 / 9.0 * kInvPi) * rsqrt(pz);
+      pref = (1.0 / 9.0 * kInvPi) * rpz;
       const double bm1 = sm1 * sp1;                      // b - 1
       if (oma < 0.5 * a) {
         // |n| = (1-a)/a < 1/2: write cK·K + cP·Π = (cK+cP)·K + cP·(Π-K) with cK+cP formed without cancellation.
@@ -134,27 +142,30 @@ __device__ __forceinline__ Basis ma_basis(double p, double z) {
         // 1/sqrt(pz) diverges: the plain form loses ~1e-16/sqrt(z) there.
         cK = fma(-bm1, 2.0 * b + a - 3.0, -3.0 * q * fma(a, bm1, oma) * (rd * rd));
         a2 = 0.0;
-        b2n = -oma * (rd * rd);                          // n = (a-1)/a
+        b2 = -oma * (rd * rd) * ad;                      // n/sp, n = (a-1)/a
       } else {
         cK = fma(-bm1, 2.0 * b + a - 3.0, -3.0 * q * (b - 2.0));
       }
     } else {
-      mc = -sm1 * sp1 / oma;
+      const double roma = rsqrt_fast(oma);
+      const double rs = rcp_fast(s);
+      mc = -sm1 * sp1 * (roma * roma);
       sp = s * fabs(rd);      // sqrt(b/a)
+      b2 = ad * rs;           // 1/sp
       cE = oma * w7;
-      pref = (2.0 / 9.0 * kInvPi) * rsqrt(oma);
+      pref = (2.0 / 9.0 * kInvPi) * roma;
       const double pz4 = 4.0 * p * z;                    // b - a
       if (pz4 < 0.5 * d * d) {
         // |n| = (b-a)/a < 1/2: same rewrite; cK = (1-a)(1-b) + 3q, so cK + cP = (1-a)[(1-b) - 3q/a]
         cK = oma * fma(-3.0 * q, rd * rd, -sm1 * sp1);
         a2 = 0.0;
-        b2n = -pz4 * (rd * rd);                          // n = (a-b)/a
+        b2 = -pz4 * (rd * rd) * (ad * rs);               // n/sp, n = (a-b)/a
       } else {
         cK = 1.0 - 5.0 * z2 + p2 + q * q;
       }
     }
   }
-  r.ld = fma(pref, cel_pair(mc, sp, cK, cE, cP, a2, b2n), add);
+  r.ld = fma(pref, cel_pair(mc, sp, cK, cE, cP, a2, b2), add);
   return r;
 }
 

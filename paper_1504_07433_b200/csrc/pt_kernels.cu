@@ -21,6 +21,9 @@
 namespace pt {
 
 constexpr int kThreads = 256;
+#ifndef PT_MIN_BLOCKS
+#define PT_MIN_BLOCKS 3   // resident blocks per SM the flux kernel is compiled for (register cap 65536/(256*PT_MIN_BLOCKS))
+#endif
 constexpr int kMaxPassbands = 1024;  // 3 doubles of shared memory each
 constexpr int kUnroll = 4;            // 32-exposure groups a warp streams per iteration (independent loads in flight)
 constexpr int kQueue = 512;           // per-warp ring queue: > 2*32*kUnroll + 32 entries, power of two
@@ -143,7 +146,7 @@ __device__ __forceinline__ void store_one_pair(OutT* __restrict__ out, int64_t n
 // warp evaluates it with all lanes busy.  Warps of a block take interleaved super-groups, so in-transit work is spread
 // over the block.
 template <int MODE, int V, bool NPB1, typename OutT>
-__global__ void __launch_bounds__(kThreads, 2) flux_kernel(const FluxArgs A) {
+__global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const FluxArgs A) {
   extern __shared__ double s_coef[];   // 3 * n_pb
   __shared__ PvConst c;
   __shared__ uint32_t s_queue[kThreads / 32][kQueue];
@@ -194,6 +197,7 @@ __global__ void __launch_bounds__(kThreads, 2) flux_kernel(const FluxArgs A) {
   const double off0 = (n_ss > 1) ? subsample_offset(g, n_ss, A.t_exp) : 0.0;
   const double inv_nss = 1.0 / (double)n_ss;
   const double khat = c.khat;
+  const bool slow_div = flags & PV_SLOWDIV;
   const double w_t0 = c.t0, w_invP = c.invP, w_mid = c.win_mid, w_half = c.win_half;
   uint32_t* queue = s_queue[warp];
   int qhead = 0, qcount = 0;   // warp-uniform
@@ -209,7 +213,7 @@ __global__ void __launch_bounds__(kThreads, 2) flux_kernel(const FluxArgs A) {
       for (int s = g; s < n_ss; s += G) {
         const double off = (s == g) ? off0 : subsample_offset(s, n_ss, A.t_exp);
         const double ts = (n_ss > 1) ? __dadd_rn(t, off) : t;
-        const double ph = fold_phase(ts, c.t0, c.P);
+        const double ph = fold_phase(ts, c.t0, c.P, c.invP, slow_div);
         const double zs = orbit_z_signed(c, ph);
         if (zs >= 0.0 && zs < 1.0 + khat) {
           Basis b;
@@ -333,7 +337,7 @@ __global__ void __launch_bounds__(kThreads) orbit_kernel(const double* __restric
       const int s = (int)(i - e * n_ss);
       const double t = __ldg(tt + e);
       const double ts = (n_ss > 1) ? __dadd_rn(t, subsample_offset(s, n_ss, t_exp)) : t;
-      z = orbit_z_signed(c, fold_phase(ts, c.t0, c.P));
+      z = orbit_z_signed(c, fold_phase(ts, c.t0, c.P, c.invP, c.flags & PV_SLOWDIV));
     }
     zo[i] = z;
   }
@@ -349,7 +353,7 @@ __global__ void __launch_bounds__(kThreads) table_kernel(double k_min, double dk
     const double k = __dadd_rn(k_min, __dmul_rn((double)i, dk));
     const double z = __dmul_rn((double)j, dz);
     Basis b;
-    if (k > 0.0) b = ma_basis(k, z);
+    if (k > 1.0e-150) b = ma_basis(k, z);
     else { b.le = 0.0; b.ld = 0.0; b.ed = 0.0; }
     TT* o = tb + idx * n_fn;
     o[0] = (TT)b.le; o[1] = (TT)b.ld; o[2] = (TT)b.ed;

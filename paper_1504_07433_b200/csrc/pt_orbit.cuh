@@ -8,11 +8,13 @@
 #include <cuda_runtime.h>
 #include <math_constants.h>
 
+#include "pt_math.cuh"
+
 namespace pt {
 
 constexpr double kTwoPi = 6.28318530717958647692;
 
-enum PvFlags : int { PV_BAD = 1, PV_CIRCULAR = 2, PV_NEVER = 4, PV_ALWAYS = 8, PV_OFF_TABLE = 16 };
+enum PvFlags : int { PV_BAD = 1, PV_CIRCULAR = 2, PV_NEVER = 4, PV_ALWAYS = 8, PV_OFF_TABLE = 16, PV_SLOWDIV = 32 };
 
 // Constants of one parameter vector (shared memory, one per block).
 struct PvConst {
@@ -26,8 +28,19 @@ struct PvConst {
 };
 
 // H1: phase fold — one subtraction, one IEEE division, round-to-nearest-even, one (exact) subtraction.
-__device__ __forceinline__ double fold_phase(double t, double t0, double P) {
-  const double x = __ddiv_rn(__dsub_rn(t, t0), P);
+// The correctly rounded quotient is obtained without the generic division sequence: with y = RN(1/P) (computed once per
+// parameter vector), q0 = RN(x y), r = x - q0 P (exact in an FMA), q = RN(q0 + r y) equals RN(x/P) for every x
+// (Markstein's theorem) unless the significand of P is all ones; that one case takes the division instruction sequence.
+__device__ __forceinline__ double fold_phase(double t, double t0, double P, double invP, bool slow_div) {
+  const double xs = __dsub_rn(t, t0);
+  double x;
+  if (slow_div) {
+    x = __ddiv_rn(xs, P);
+  } else {
+    const double q0 = __dmul_rn(xs, invP);
+    const double r = __fma_rn(-q0, P, xs);
+    x = __fma_rn(r, invP, q0);
+  }
   return __dsub_rn(x, rint(x));
 }
 
@@ -55,21 +68,23 @@ __device__ __forceinline__ bool in_window(double t, double t0, double invP, doub
 // root so Newton descends monotonically (<= 12 steps at e = 0.999).
 __device__ __forceinline__ void kepler_newton(double M, double e, double* sinE, double* cosE) {
   double E;
+  double sE, cE, dE;
   if (e <= 0.8) {
-    const double sM = sin(M);
-    E = M + e * sM / (1.0 - sin(M + e) + sM);
+    double sM, cM, sMe, cMe;
+    sincos_bounded(M, &sM, &cM);
+    sincos_bounded(M + e, &sMe, &cMe);
+    E = fma(e * sM, rcp_fast(1.0 - sMe + sM), M);
   } else {
     E = M + copysign(e, M);
   }
-  double sE, cE, dE;
   const double tol = 1.0e-9 * (1.0 - e);
   bool conv = false;
 #pragma unroll 1
   for (int it = 0; it < 32; ++it) {
-    sincos(E, &sE, &cE);
-    const double f = E - e * sE - M;
-    const double fp = 1.0 - e * cE;
-    dE = f / fp;
+    sincos_bounded(E, &sE, &cE);
+    const double f = E - fma(e, sE, M);
+    const double fp = fma(-e, cE, 1.0);
+    dE = f * rcp_fast(fp);
     E -= dE;
     if (fabs(dE) < tol) { conv = true; break; }   // the step just applied squares the error: converged to rounding
   }
@@ -77,7 +92,7 @@ __device__ __forceinline__ void kepler_newton(double M, double e, double* sinE, 
     *sinE = fma(-cE, dE, sE);
     *cosE = fma(sE, dE, cE);
   } else {
-    sincos(E, sinE, cosE);
+    sincos_bounded(E, sinE, cosE);
   }
 }
 
@@ -85,9 +100,9 @@ __device__ __forceinline__ void kepler_newton(double M, double e, double* sinE, 
 __device__ __forceinline__ double orbit_z_signed(const PvConst& c, double ph) {
   if (c.flags & PV_CIRCULAR) {
     double sn, cs;
-    sincospi(2.0 * ph, &sn, &cs);
+    sincos_bounded(kTwoPi * ph, &sn, &cs);
     const double cc = c.cosi * cs;
-    const double z = c.a * sqrt(fma(sn, sn, cc * cc));
+    const double z = c.a * sqrt_fast(fmax(fma(sn, sn, cc * cc), 1.0e-300));
     return cs > 0.0 ? z : -z;
   }
   double M = fma(kTwoPi, ph, c.Mtr);
@@ -99,7 +114,7 @@ __device__ __forceinline__ double orbit_z_signed(const PvConst& c, double ph) {
   const double A = c.cosw * x - c.sinw * y;   // (r/a) cos(w+f)
   const double B = c.sinw * x + c.cosw * y;   // (r/a) sin(w+f)
   const double Bc = B * c.cosi;
-  const double z = c.a * sqrt(fma(A, A, Bc * Bc));
+  const double z = c.a * sqrt_fast(fmax(fma(A, A, Bc * Bc), 1.0e-300));
   return B > 0.0 ? z : -z;
 }
 
@@ -121,7 +136,8 @@ __device__ inline void pv_setup_orbit(PvConst& c, const double* row, bool row_ok
     c.flags = PV_BAD;
     return;
   }
-  c.t0 = t0; c.P = P; c.invP = 1.0 / P; c.a = a; c.e = e;
+  c.t0 = t0; c.P = P; c.invP = __drcp_rn(P); c.a = a; c.e = e;
+  if ((__double_as_longlong(P) & 0x000fffffffffffffLL) == 0x000fffffffffffffLL) flags |= PV_SLOWDIV;
   c.cosi = cos(inc);
   const double k = c.khat;
   const double margin = 1.0e-7;   // cycles; the cheap fold differs from the pinned one by < 2.3e-16 |x| <= 2.3e-8
@@ -167,7 +183,7 @@ __device__ inline void pv_setup_orbit(PvConst& c, const double* row, bool row_ok
       if (!(hi < 0.45 && lo > -0.45)) { flags |= PV_ALWAYS; lo = -1.0; hi = 1.0; }   // folded phase must not wrap
     }
   }
-  if (!(k > 0.0)) { flags |= PV_NEVER; }
+  if (!(k > 1.0e-150)) { flags |= PV_NEVER; }
   c.ph_lo = lo; c.ph_hi = hi;
   const double hx = (n_ss > 1) ? fabs(0.5 * t_exp * c.invP) * (1.0 + 1.0e-9) : 0.0;
   c.ex_lo = lo - hx; c.ex_hi = hi + hx;
