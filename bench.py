@@ -114,7 +114,8 @@ def _barrier(world: int):
     if world > 1:
         import torch.distributed as dist
         dist.barrier()
-    torch.cuda.synchronize()
+    if torch.cuda.is_available():
+        torch.cuda.synchronize()
 
 
 def _time_steps(fn, steps: int, warmup: int, flush, world: int):
