@@ -17,9 +17,6 @@ struct Basis {
   double le, ld, ed;
 };
 
-constexpr double kPi = 3.14159265358979323846;
-constexpr double kInvPi = 0.31830988618379067154;
-constexpr double kTwoThirds = 0.66666666666666666667;
 
 // cK·K(m) + cE·E(m) + cP·cel(kc, 1-n, a2, b2·sp) with mc = 1-m = kc² and sp = sqrt(1-n) > 0 the square root of the second
 // sequence's p-argument.  (a2, b2) = (1, 1/sp) makes the second integral Π(n|m); (0, n/sp) makes it Π(n|m) - K(m).
@@ -51,7 +48,7 @@ __device__ __forceinline__ double cel_pair(double mc, double sp, double cK, doub
     // ladder
     const double g = em;
     em += qc;
-    if (fabs(g - qc) <= 1.0e-8 * g) break;
+    if (fabs(g - qc) <= 0x1p-27 * g) break;   // 7.5e-9: the next step squares it
     qc = 2.0 * sqrt_fast(e);
     e = qc * em;
   }
@@ -59,13 +56,13 @@ __device__ __forceinline__ double cel_pair(double mc, double sp, double cK, doub
   const double rr = rcp_fast(d1 * d2);
   const double s1 = fma(a1, em, b1) * (d2 * rr);
   const double s2 = fma(a2, em, b2) * (d1 * rr);
-  return (0.5 * kPi) * fma(cP, s2, s1);
+  return kC[C_HALFPI] * fma(cP, s2, s1);
 }
 
 // Basis functions at radius ratio p > 0 and separation z >= 0 (planet in front of the star).
 __device__ __forceinline__ Basis ma_basis(double p, double z) {
   Basis r;
-  z = fmax(z, 1.0e-150);   // keeps every operand of the fast reciprocals normal; changes nothing above 1e-150
+  z = fmax(z, 0x1p-500);   // 3e-151: keeps every operand of the fast reciprocals normal; changes nothing above it
   // d = z-p, s = z+p and the four contact distances 1-d, 1+d, s-1, s+1.  Each is formed so that the operand pair that
   // nearly cancels at "its" contact is subtracted exactly first (Sterbenz), e.g. s-1 = z + (p-1) for p in [1/2, 2]:
   // a plain (z+p)-1 loses z entirely when z << p ~ 1 (and mc = (s-1)(s+1)/(4zp) then has O(1) relative error).
@@ -77,7 +74,7 @@ __device__ __forceinline__ Basis ma_basis(double p, double z) {
   const double omd = (p < 1.0) ? (1.0 - z) + p : 1.0 - d;                    // 1 - d
   const double sp1 = s + 1.0;
   if (omd <= 0.0) { r.le = 0.0; r.ld = 0.0; r.ed = 0.0; return r; }                  // no overlap (z >= 1+p)
-  if (opd <= 0.0) { r.le = 1.0; r.ld = kTwoThirds; r.ed = 0.5; return r; }           // star covered (z <= p-1)
+  if (opd <= 0.0) { r.le = 1.0; r.ld = kC[C_TWOTHIRDS]; r.ed = 0.5; return r; }           // star covered (z <= p-1)
   const double p2 = p * p, z2 = z * z;
   const double eta2 = 0.5 * p2 * fma(2.0, z2, p2);
   const double oma = omd * opd;                // 1 - a
@@ -86,24 +83,24 @@ __device__ __forceinline__ Basis ma_basis(double p, double z) {
   if (partial) {
     const double T = sqrt_fast(oma * sm1 * sp1);
     const double pp1 = pm1 * (p + 1.0);                  // p² - 1 without cancellation for p ~ 1
-    const double kap0 = atan2(T, z2 + pp1);
-    const double kap1 = atan2(T, z2 - pp1);
-    r.le = (fma(p2, kap0, kap1) - 0.5 * T) * kInvPi;
-    r.ed = (fma(2.0 * eta2, kap0, kap1) - 0.25 * (1.0 + 5.0 * p2 + z2) * T) * (0.5 * kInvPi);
+    const double kap0 = atan2_pos(T, z2 + pp1);
+    const double kap1 = atan2_pos(T, z2 - pp1);
+    r.le = (fma(p2, kap0, kap1) - 0.5 * T) * kC[C_INVPI];
+    r.ed = (fma(2.0 * eta2, kap0, kap1) - 0.25 * (1.0 + 5.0 * p2 + z2) * T) * kC[C_HALF_INVPI];
   } else {
     r.le = p2;
     r.ed = eta2;
   }
 
   if (sm1 == 0.0) {  // inner contact z = 1-p: elementary closed form (exact equality only; table nodes land here)
-    r.ld = (2.0 / 3.0 * kInvPi) * acos(1.0 - 2.0 * p) - (4.0 / 9.0 * kInvPi) * (3.0 + 2.0 * p - 8.0 * p2) * sqrt(p * (1.0 - p));  // rare branch: library sqrt/acos are fine here
+    r.ld = (2.0 / 3.0 * kC[C_INVPI]) * acos(1.0 - 2.0 * p) - (4.0 / 9.0 * kC[C_INVPI]) * (3.0 + 2.0 * p - 8.0 * p2) * sqrt(p * (1.0 - p));  // rare branch: library sqrt/acos are fine here
     return r;
   }
 
   double mc, sp, cK, cE, cP, pref, add;
   double a2 = 1.0, b2;
-  if (fabs(d) < 1.0e-100) {  // z = p: the Π term drops out
-    add = 1.0 / 3.0;
+  if (fabs(d) < 0x1p-332) {  // 1e-100  // z = p: the Π term drops out
+    add = kC[C_THIRD];
     cP = 0.0;
     sp = 1.0;
     b2 = 1.0;
@@ -111,20 +108,20 @@ __device__ __forceinline__ Basis ma_basis(double p, double z) {
       mc = (1.0 - 2.0 * p) * (1.0 + 2.0 * p);
       cE = 4.0 * (2.0 * p2 - 1.0);
       cK = mc;
-      pref = 2.0 / 9.0 * kInvPi;
+      pref = kC[C_2INV9PI];
     } else {  // p > 1/2, m = 1/(4p²)
       const double i4p2 = rcp_fast(4.0 * p2);
       mc = (2.0 * p - 1.0) * (2.0 * p + 1.0) * i4p2;
       cE = 16.0 * p * (2.0 * p2 - 1.0);
       cK = -(1.0 - 4.0 * p2) * (3.0 - 8.0 * p2) * rcp_fast(p);
-      pref = 1.0 / 9.0 * kInvPi;
+      pref = kC[C_INV9PI];
     }
   } else {
     const double rd = rcp_fast(d);
     const double ad = fabs(d);
     const double q = -d * s;  // p² - z²
     const double w7 = z2 + 7.0 * p2 - 4.0;
-    add = d < 0.0 ? kTwoThirds : 0.0;
+    add = d < 0.0 ? kC[C_TWOTHIRDS] : 0.0;
     cP = 3.0 * s * rd;        // -3q/a
     if (partial) {
       const double a = d * d, b = s * s;
@@ -134,7 +131,7 @@ __device__ __forceinline__ Basis ma_basis(double p, double z) {
       sp = fabs(rd);          // sqrt(1/a)
       b2 = ad;                // 1/sp
       cE = 4.0 * pz * w7;
-      pref = (1.0 / 9.0 * kInvPi) * rpz;
+      pref = kC[C_INV9PI] * rpz;
       const double bm1 = sm1 * sp1;                      // b - 1
       if (oma < 0.5 * a) {
         // |n| = (1-a)/a < 1/2: write cK·K + cP·Π = (cK+cP)·K + cP·(Π-K) with cK+cP formed without cancellation.
@@ -153,7 +150,7 @@ __device__ __forceinline__ Basis ma_basis(double p, double z) {
       sp = s * fabs(rd);      // sqrt(b/a)
       b2 = ad * rs;           // 1/sp
       cE = oma * w7;
-      pref = (2.0 / 9.0 * kInvPi) * roma;
+      pref = kC[C_2INV9PI] * roma;
       const double pz4 = 4.0 * p * z;                    // b - a
       if (pz4 < 0.5 * d * d) {
         // |n| = (b-a)/a < 1/2: same rewrite; cK = (1-a)(1-b) + 3q, so cK + cP = (1-a)[(1-b) - 3q/a]

@@ -283,15 +283,19 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const Flu
         }
       }
     }
-    if (__any_sync(0xffffffffu, inw != 0)) {
-#pragma unroll
-      for (int uv = 0; uv < kUnroll * V; ++uv) {
+    // append the in-window exposures to the ring queue: one ballot per (u,v) slot that has any taker in the warp
+    // (REDUX.OR finds those slots in one instruction; typically 0-2 of the kUnroll*V are non-empty)
+    unsigned slots = __reduce_or_sync(0xffffffffu, inw);
+    if (slots) {
+      const unsigned lt = (1u << lane) - 1u;
+      do {
+        const int uv = __ffs(slots) - 1;
+        slots &= slots - 1u;
         const bool b = (inw >> uv) & 1u;
         const unsigned m = __ballot_sync(0xffffffffu, b);
-        if (b) queue[(qhead + qcount + __popc(m & ((1u << lane) - 1u))) & (kQueue - 1)] =
-            base + ((uv / V) * 32 + lane) * V + (uv % V);
+        if (b) queue[(qhead + qcount + __popc(m & lt)) & (kQueue - 1)] = base + ((uv / V) * 32 + lane) * V + (uv % V);
         qcount += __popc(m);
-      }
+      } while (slots);
       __syncwarp();
     }
     const bool last = (it + 1 == n_iter);

@@ -12,7 +12,8 @@
 
 namespace pt {
 
-constexpr double kTwoPi = 6.28318530717958647692;
+constexpr double kTwoPi = 6.28318530717958647692;   // host-side / setup use; hot paths read kC[]
+constexpr double kPi = 3.14159265358979323846;
 
 enum PvFlags : int { PV_BAD = 1, PV_CIRCULAR = 2, PV_NEVER = 4, PV_ALWAYS = 8, PV_OFF_TABLE = 16, PV_SLOWDIV = 32 };
 
@@ -60,7 +61,7 @@ __device__ __forceinline__ bool in_window(double t, double t0, double invP, doub
   const double magic = 6755399441055744.0;   // 1.5 * 2^52
   const double r = __dsub_rn(__dadd_rn(x, magic), magic);
   const double ph = x - r;
-  return fabs(ph - mid) < fma(fabs(x), 1.0e-15, half);
+  return fabs(ph - mid) < fma(fabs(x), 0x1p-50, half);
 }
 
 // Eccentric anomaly from mean anomaly M in (-π, π] by Newton's method.  Starter: for e <= 0.8 the third-order
@@ -77,7 +78,7 @@ __device__ __forceinline__ void kepler_newton(double M, double e, double* sinE, 
   } else {
     E = M + copysign(e, M);
   }
-  const double tol = 1.0e-9 * (1.0 - e);
+  const double tol = 0x1p-30 * (1.0 - e);
   bool conv = false;
 #pragma unroll 1
   for (int it = 0; it < 32; ++it) {
@@ -100,21 +101,21 @@ __device__ __forceinline__ void kepler_newton(double M, double e, double* sinE, 
 __device__ __forceinline__ double orbit_z_signed(const PvConst& c, double ph) {
   if (c.flags & PV_CIRCULAR) {
     double sn, cs;
-    sincos_bounded(kTwoPi * ph, &sn, &cs);
+    sincos_bounded(kC[C_TWOPI] * ph, &sn, &cs);
     const double cc = c.cosi * cs;
-    const double z = c.a * sqrt_fast(fmax(fma(sn, sn, cc * cc), 1.0e-300));
+    const double z = c.a * sqrt_fast(fmax(fma(sn, sn, cc * cc), 0x1p-1000));
     return cs > 0.0 ? z : -z;
   }
-  double M = fma(kTwoPi, ph, c.Mtr);
-  if (M > kPi) M -= kTwoPi;
-  if (M <= -kPi) M += kTwoPi;
+  double M = fma(kC[C_TWOPI], ph, c.Mtr);
+  if (M > kC[C_PI]) M -= kC[C_TWOPI];
+  if (M <= -kC[C_PI]) M += kC[C_TWOPI];
   double sE, cE;
   kepler_newton(M, c.e, &sE, &cE);
   const double x = cE - c.e, y = c.rt1me2 * sE;
   const double A = c.cosw * x - c.sinw * y;   // (r/a) cos(w+f)
   const double B = c.sinw * x + c.cosw * y;   // (r/a) sin(w+f)
   const double Bc = B * c.cosi;
-  const double z = c.a * sqrt_fast(fmax(fma(A, A, Bc * Bc), 1.0e-300));
+  const double z = c.a * sqrt_fast(fmax(fma(A, A, Bc * Bc), 0x1p-1000));
   return B > 0.0 ? z : -z;
 }
 
