@@ -1,0 +1,617 @@
+// pt_flux.cuh — the fused flux kernel: S0-S7 (and S9) of the hot path in one persistent launch.
+//
+// Every warp is an autonomous pipeline; the block is only a container (no block barrier anywhere).  A warp takes tiles
+// (parameter vector pv, run of `tile_len` exposures) in a strided order and pushes the work through three stages, each of
+// which runs with (nearly) all 32 lanes busy because the stages are decoupled by per-warp queues in shared memory:
+//
+//   stream   every exposure of the tile: 16-byte time loads, a 6-instruction phase-window test, flux = 1 written with
+//            16-byte streaming stores for the exposures that cannot be in transit; the others go to the EXPOSURE queue
+//   z-stage  G = min(n_ss,32) lanes per queued exposure: pinned subsample time + phase fold (H1, H2), orbit -> signed z
+//            (Newton–Kepler for e > 0).  Subsamples with 0 <= z < 1+k̂ are compacted (ballot + popc, order kept) into
+//            the ITEM queue; an exposure without any such subsample is finished here (flux = 1)
+//   basis    32 queued subsamples, possibly of different exposures, tiles and parameter vectors: λe, λd*, ηd by the closed
+//            forms / one shared `cel` ladder (pt_basis.cuh) or the bilinear table lookup; the supersample sum is a
+//            segmented warp-shuffle reduction over the lanes that belong to one exposure, in 64-bit fixed point so that
+//            the result does not depend on how an exposure's subsamples were split over batches (integer addition is
+//            associative: bit-reproducible whatever the queue history); the last subsample of an exposure applies the
+//            limb-darkening combine per passband and stores.
+//
+// This is the "binning" BASELINE.json asks for: the expensive stage only ever sees in-transit subsamples, 32 at a time,
+// and inside/partial lanes differ only in the coefficients they feed to the shared elliptic-integral loop.  Queues
+// survive tile changes (items carry the index of a small per-warp ring of parameter-vector records), so small tiles —
+// needed to balance a small problem over 148 SMs — do not leave ragged batches behind.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/pt.h"
+#include "pt_basis.cuh"
+#include "pt_orbit.cuh"
+
+namespace pt {
+
+constexpr int kThreads = 256;
+constexpr int kWarpsPerBlock = kThreads / 32;
+#ifndef PT_MIN_BLOCKS
+#define PT_MIN_BLOCKS 3   // resident blocks per SM the flux kernel is compiled for (register cap 65536/(256*PT_MIN_BLOCKS))
+#endif
+constexpr int kMaxPassbands = 1024;
+constexpr int kUnroll = 4;      // 32-exposure groups a warp streams per iteration (independent loads in flight)
+constexpr int kExpQ = 512;      // exposure ring: >= 32*kUnroll*2 + 32 entries, power of two, uint16 tile-local indices
+constexpr int kItemQ = 64;      // item ring: at most 31 left over + 32 new per z-round
+constexpr int kSlots = 64;      // pending-exposure records (supersampled path): <= 31 + 32 alive
+constexpr int kPvRing = 4;      // parameter-vector records a warp keeps alive (single-passband path)
+constexpr int kCoefCache = 32;  // passbands whose combine coefficients are cached per warp (multi-passband path)
+constexpr int kMaxTileLen = 32768;
+constexpr int kRemBias = 1 << 24;
+
+struct FluxArgs {
+  const double* times;
+  int64_t n_t, t_stride_pv;
+  const double* params;
+  int64_t n_pv;
+  int n_pb, n_ss;
+  double t_exp;
+  void* flux;
+  int32_t* status;
+  // tiling
+  int tile_len;            // exposures per tile (multiple of 256, <= kMaxTileLen)
+  int tiles_per_pv;
+  int64_t n_tiles;
+  // supersample accumulation (fixed point)
+  int fx_bits;             // 61 - ceil(log2 n_ss): a sum of n_ss values below 2^eb fits an int64 at scale 2^(fx_bits-eb)
+  double fx_scale;         // 2^fx_bits (basis values are <= 1)
+  double fx_inv;           // 1 / (fx_scale * n_ss)
+  // interpolation table (mode 1)
+  const void* tb;
+  int tb_dtype, n_k, n_z, n_fn;
+  double k_min, dk, dz;
+};
+
+__device__ __forceinline__ double nan64() { return __longlong_as_double(0x7ff8000000000000LL); }
+
+// One parameter vector as a warp sees it while a tile of it is being streamed, and for as long as queued subsamples of
+// that tile are alive.
+struct PvRec {
+  PvConst c;               // orbit constants, k̂, phase window (pt_orbit.cuh)
+  const double* tb;        // times of the tile
+  char* ob;                // flux of the tile: row pv, passband 0, first exposure of the tile
+  double coef[3];          // single passband: g(1-c)/N, g c/N, g u2/N
+  double acc_scale;        // single passband: fixed-point scale of the combined decrement, and its inverse / n_ss
+  double acc_inv;
+  double ik2;              // 1/k̂² (0 when k̂ == 0)
+  const double* row;       // parameter row (multi-passband combine beyond the coefficient cache)
+  double w_c0, w_half;     // cheap window test: x' = t*invP + w_c0, |x' - rint(x')| < w_half + 2^-50 |x'|
+  double fk;               // table: fractional k index
+  int ik;                  // table: lower k index
+  int use_table;
+};
+
+struct Slot {              // a supersampled exposure with subsamples still in the item queue
+  long long acc[3];        // fixed-point sums (single passband: acc[0] = combined decrement)
+  int remaining;           // subsamples not yet evaluated (+ kRemBias while the exposure is still being expanded)
+  uint16_t e;              // tile-local exposure index
+  uint16_t ring;           // PvRec index
+};
+
+struct WarpState {
+  PvRec pv[kPvRing];
+  Slot slots[kSlots];
+  double item_z[kItemQ];
+  uint16_t item_tag[kItemQ];    // supersampled: slot index; n_ss == 1: tile-local exposure index
+  uint8_t item_ring[kItemQ];    // n_ss == 1: PvRec index
+  uint16_t expq[kExpQ];
+  double coefc[3 * kCoefCache];
+  int qhead, qcount;            // exposure ring
+  int ihead, icount;            // item ring
+  int slot_next;                // next slot to hand out (mod kSlots)
+  int cur;                      // PvRec of the tile being streamed
+};
+
+template <typename OutT> struct Vec2;
+template <> struct Vec2<double> { typedef double2 type; };
+template <> struct Vec2<float> { typedef float2 type; };
+
+// flux = 1 for one exposure / an aligned pair of exposures, all passbands (streaming stores: the output is write-once).
+template <bool NPB1, typename OutT>
+__device__ __forceinline__ void store_one(OutT* __restrict__ out, int64_t n_t, int n_pb) {
+  if (NPB1) __stcs(out, (OutT)1.0);
+  else for (int j = 0; j < n_pb; ++j) __stcs(out + (int64_t)j * n_t, (OutT)1.0);
+}
+template <bool NPB1, typename OutT>
+__device__ __forceinline__ void store_one_pair(OutT* __restrict__ out, int64_t n_t, int n_pb) {
+  typename Vec2<OutT>::type v;
+  v.x = (OutT)1.0; v.y = (OutT)1.0;
+  if (NPB1) __stcs((typename Vec2<OutT>::type*)out, v);
+  else for (int j = 0; j < n_pb; ++j) __stcs((typename Vec2<OutT>::type*)(out + (int64_t)j * n_t), v);
+}
+
+// Limb-darkening combine (Eq. 13 with the k-correction of P:L179) of one exposure's mean basis functions, and the
+// stores.  Single passband: the decrement arrives already combined in `le`.
+template <bool NPB1, typename OutT>
+__device__ __forceinline__ void finish_exposure(const FluxArgs& A, const WarpState& ws, const PvRec& r, uint32_t e,
+                                                double le, double ld, double ed) {
+  OutT* out = (OutT*)r.ob + e;
+  if (NPB1) {
+    __stcs(out, (OutT)(1.0 - le));
+  } else {
+    const int n_pb = A.n_pb;
+    const int nc = n_pb < kCoefCache ? n_pb : kCoefCache;
+    for (int j = 0; j < nc; ++j) {
+      const double v = 1.0 - fma(ws.coefc[3 * j + 2], ed, fma(ws.coefc[3 * j + 1], ld, ws.coefc[3 * j] * le));
+      __stcs(out + (int64_t)j * A.n_t, (OutT)v);
+    }
+    for (int j = nc; j < n_pb; ++j) {   // beyond the cache: coefficients from the parameter row
+      const double k = __ldg(r.row + 6 + 3 * j), u1 = __ldg(r.row + 7 + 3 * j), u2 = __ldg(r.row + 8 + 3 * j);
+      const double cj = u1 + 2.0 * u2;
+      const double gN = k * k * r.ik2 / (1.0 - u1 / 3.0 - u2 / 6.0);
+      const double v = 1.0 - fma(gN * u2, ed, fma(gN * cj, ld, gN * (1.0 - cj) * le));
+      __stcs(out + (int64_t)j * A.n_t, (OutT)v);
+    }
+  }
+}
+
+// Bilinear lookup of the three functions.  Corner loads go through the read-only path; the table is
+// expected to live in L2.
+template <typename TT>
+__device__ __forceinline__ Basis table_lookup(const FluxArgs& A, int ik, double fk, double z) {
+  const double rz = z / A.dz;
+  int iz = (int)floor(rz);
+  iz = min(max(iz, 0), A.n_z - 2);
+  const double fz = rz - (double)iz;
+  const TT* r0 = (const TT*)A.tb + ((size_t)ik * A.n_z + iz) * A.n_fn;
+  const TT* r1 = r0 + (size_t)A.n_z * A.n_fn;
+  double v[3];
+#pragma unroll
+  for (int f = 0; f < 3; ++f) {
+    const double t00 = (double)__ldg(r0 + f), t01 = (double)__ldg(r0 + A.n_fn + f);
+    const double t10 = (double)__ldg(r1 + f), t11 = (double)__ldg(r1 + A.n_fn + f);
+    const double lo = fma(fz, t01 - t00, t00);
+    const double hi = fma(fz, t11 - t10, t10);
+    v[f] = fma(fk, hi - lo, lo);
+  }
+  Basis b;
+  b.le = v[0]; b.ld = v[1]; b.ed = v[2];
+  return b;
+}
+
+template <int MODE>
+__device__ __forceinline__ Basis eval_basis(const FluxArgs& A, const PvRec& r, double z) {
+  if (MODE == 1 && r.use_table)
+    return (A.tb_dtype == PT_F64) ? table_lookup<double>(A, r.ik, r.fk, z) : table_lookup<float>(A, r.ik, r.fk, z);
+  return ma_basis(r.c.khat, z);
+}
+
+// 2^s as a double, s clamped to the normal range.
+__device__ __forceinline__ double pow2i(int s) {
+  s = min(max(s, -1000), 1000);
+  return __longlong_as_double((long long)(s + 1023) << 52);
+}
+
+// S0: per-tile setup, executed redundantly by all lanes of the warp (same cost as one lane; lane 0 writes).
+// Row validation, k̂ (summed in index order, R9), orbit constants and phase window (pv_setup_orbit), combine
+// coefficients coef = g (1-c)/N, g c/N, g u2/N with g = k_j²/k̂², table indices, window-test constants.
+template <int MODE, bool NPB1, typename OutT>
+__device__ __noinline__ void tile_setup(const FluxArgs& A, WarpState& ws, int ring, int64_t tile) {
+  const int lane = threadIdx.x & 31;
+  PvRec& r = ws.pv[ring];
+  const int64_t pv = tile / A.tiles_per_pv;
+  const int chunk = (int)(tile - pv * A.tiles_per_pv);
+  const int n_pb = NPB1 ? 1 : A.n_pb;
+  const double* row = A.params + pv * (6 + 3 * (int64_t)n_pb);
+  bool ok = true;
+  double ksum = 0.0;
+  for (int j = 0; j < n_pb; ++j) {
+    const double k = __ldg(row + 6 + 3 * j), u1 = __ldg(row + 7 + 3 * j), u2 = __ldg(row + 8 + 3 * j);
+    const double N = 1.0 - u1 / 3.0 - u2 / 6.0;
+    if (!(isfinite(k) && isfinite(u1) && isfinite(u2)) || !(k >= 0.0) || N == 0.0) ok = false;
+    ksum += k;
+  }
+  const double khat = ksum / (double)n_pb;
+  PvConst c;
+  c.khat = khat;
+  pv_setup_orbit(c, row, ok, A.n_ss, A.t_exp);
+  const int64_t e0 = (int64_t)chunk * A.tile_len;
+  const double ik2 = khat > 0.0 ? 1.0 / (khat * khat) : 0.0;
+  if (lane == 0) {
+    r.c = c;
+    r.tb = A.times + pv * A.t_stride_pv + e0;
+    r.ob = (char*)A.flux + ((pv * n_pb) * A.n_t + e0) * (int64_t)sizeof(OutT);
+    r.row = row;
+    r.ik2 = ik2;
+    r.use_table = 0;
+  }
+  if (c.flags & PV_BAD) {
+    if (chunk == 0 && lane == 0 && A.status) {
+      atomicOr(&A.status[0], PT_ST_BAD_PARAM);
+      atomicAdd(&A.status[1], 1);
+    }
+    __syncwarp();
+    return;
+  }
+  if (NPB1) {
+    const double k = __ldg(row + 6), u1 = __ldg(row + 7), u2 = __ldg(row + 8);
+    const double cj = u1 + 2.0 * u2;
+    const double gN = k * k * ik2 / (1.0 - u1 / 3.0 - u2 / 6.0);
+    const double c0 = gN * (1.0 - cj), c1 = gN * cj, c2 = gN * u2;
+    // fixed-point scale of the combined decrement c0 λe + c1 λd + c2 ηd (each basis value <= 1): 2^eb > |c0|+|c1|+|c2|
+    const double B = fabs(c0) + fabs(c1) + fabs(c2);
+    int eb = (int)((__double_as_longlong(B) >> 52) & 0x7ff) - 1022;
+    if (!(B > 0.0) || !isfinite(B)) eb = 0;
+    const double sc = pow2i(A.fx_bits - eb);
+    if (lane == 0) {
+      r.coef[0] = c0; r.coef[1] = c1; r.coef[2] = c2;
+      r.acc_scale = sc;
+      r.acc_inv = 1.0 / (sc * (double)A.n_ss);
+    }
+  } else {
+    for (int j = lane; j < n_pb && j < kCoefCache; j += 32) {
+      const double k = __ldg(row + 6 + 3 * j), u1 = __ldg(row + 7 + 3 * j), u2 = __ldg(row + 8 + 3 * j);
+      const double cj = u1 + 2.0 * u2;
+      const double gN = k * k * ik2 / (1.0 - u1 / 3.0 - u2 / 6.0);
+      ws.coefc[3 * j + 0] = gN * (1.0 - cj);
+      ws.coefc[3 * j + 1] = gN * cj;
+      ws.coefc[3 * j + 2] = gN * u2;
+    }
+  }
+  if (MODE == 1) {
+    const double rk = (khat - A.k_min) / A.dk;
+    const bool use_table = (khat >= A.k_min) && (khat <= A.k_min + (A.n_k - 1) * A.dk);
+    const int ik = min(max((int)floor(rk), 0), A.n_k - 2);
+    if (lane == 0) {
+      r.use_table = use_table ? 1 : 0;
+      r.ik = ik;
+      r.fk = rk - (double)ik;
+    }
+    if (!use_table && !(c.flags & PV_NEVER) && chunk == 0 && lane == 0 && A.status) {
+      atomicOr(&A.status[0], PT_ST_K_OUT_OF_TABLE);
+      atomicAdd(&A.status[1], 1);
+    }
+  }
+  // cheap window test (see in_window2): x' = t*invP + c0 approximates (t-t0)/P - mid with an error below
+  // 2^-53 (2|x'| + 2|t0/P| + 2|mid|); the test widens the half-width by 2^-50 (|x'| + |t0/P| + |mid| + 1).
+  const double t0p = c.t0 * c.invP;
+  if (lane == 0) {
+    r.w_c0 = -t0p - c.win_mid;
+    r.w_half = c.win_half + 0x1p-50 * (fabs(t0p) + fabs(c.win_mid) + 1.0);
+  }
+  __syncwarp();
+}
+
+// Cheap window test on an exposure time: can any subsample of it be in transit?  It is only ever used to SKIP exposures
+// whose flux is exactly 1, so it must never say "no" wrongly; the half-width carries the error bound of the cheap fold
+// (tile_setup) on top of the 1e-7-cycle margin built into the window.  |x'| >= 2^51: the widened half-width exceeds 2,
+// so the test passes whatever the rounding did; NaN/inf times fail it (flux 1, as in the oracle, where every comparison
+// with NaN is false).  6 FP64-pipe instructions per exposure.
+__device__ __forceinline__ bool in_window2(double t, double invP, double c0, double half) {
+  const double x = fma(t, invP, c0);
+  const double magic = 6755399441055744.0;   // 1.5 * 2^52
+  const double r = __dsub_rn(__dadd_rn(x, magic), magic);
+  const double d = x - r;
+  return fabs(d) < fma(fabs(x), 0x1p-50, half);
+}
+
+// ---------------------------------------------------------------------------------------------------- basis stage
+// Evaluate the first n (<= 32) queued subsamples, one per lane.
+template <int MODE, bool NPB1, bool SS1, typename OutT>
+__device__ __noinline__ void basis_round(const FluxArgs& A, WarpState& ws, int n) {
+  const int lane = threadIdx.x & 31;
+  const bool act = lane < n;
+  const int ihead = ws.ihead;
+  const int idx = (ihead + lane) & (kItemQ - 1);
+  if (SS1) {
+    if (act) {
+      const double z = ws.item_z[idx];
+      const uint32_t e = ws.item_tag[idx];
+      const PvRec& r = ws.pv[ws.item_ring[idx]];
+      const Basis b = eval_basis<MODE>(A, r, z);
+      if (NPB1) finish_exposure<true, OutT>(A, ws, r, e, fma(r.coef[2], b.ed, fma(r.coef[1], b.ld, r.coef[0] * b.le)), 0.0, 0.0);
+      else finish_exposure<false, OutT>(A, ws, r, e, b.le, b.ld, b.ed);
+    }
+  } else {
+    constexpr int NACC = NPB1 ? 1 : 3;
+    const int sid = act ? (int)ws.item_tag[idx] : -1 - lane;   // inactive lanes: unique ids, never equal to a neighbour's
+    long long v[NACC];
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) v[a] = 0;
+    int ring = 0;
+    if (act) {
+      ring = ws.slots[sid].ring;
+      const PvRec& r = ws.pv[ring];
+      const Basis b = eval_basis<MODE>(A, r, ws.item_z[idx]);
+      if (NPB1) {
+        v[0] = __double2ll_rn(fma(r.coef[2], b.ed, fma(r.coef[1], b.ld, r.coef[0] * b.le)) * r.acc_scale);
+      } else {
+        v[0] = __double2ll_rn(b.le * A.fx_scale);
+        v[NACC - 2] = __double2ll_rn(b.ld * A.fx_scale);
+        v[NACC - 1] = __double2ll_rn(b.ed * A.fx_scale);
+      }
+    }
+    // segmented inclusive scan over runs of equal slot id (an exposure's subsamples are contiguous in the queue)
+    const int G = A.n_ss < 32 ? A.n_ss : 32;
+    for (int o = 1; o < G; o <<= 1) {
+      const int so = __shfl_up_sync(0xffffffffu, sid, o);
+      const bool take = (lane >= o) && (so == sid);
+#pragma unroll
+      for (int a = 0; a < NACC; ++a) {
+        const long long t = __shfl_up_sync(0xffffffffu, v[a], o);
+        if (take) v[a] += t;
+      }
+    }
+    const int sprev = __shfl_up_sync(0xffffffffu, sid, 1);
+    const int snext = __shfl_down_sync(0xffffffffu, sid, 1);
+    const unsigned heads = __ballot_sync(0xffffffffu, lane == 0 || sprev != sid);
+    const bool tail = act && (lane == 31 || snext != sid);
+    if (tail) {
+      const int head = 31 - __clz(heads & (0xffffffffu >> (31 - lane)));
+      Slot& s = ws.slots[sid];
+      const int rem = s.remaining - (lane - head + 1);
+      if (rem == 0) {
+        const PvRec& r = ws.pv[ring];
+        if (NPB1) {
+          finish_exposure<true, OutT>(A, ws, r, s.e, (double)(s.acc[0] + v[0]) * r.acc_inv, 0.0, 0.0);
+        } else {
+          finish_exposure<false, OutT>(A, ws, r, s.e, (double)(s.acc[0] + v[0]) * A.fx_inv,
+                                       (double)(s.acc[NACC - 2] + v[NACC - 2]) * A.fx_inv,
+                                       (double)(s.acc[NACC - 1] + v[NACC - 1]) * A.fx_inv);
+        }
+      } else {
+        s.remaining = rem;
+#pragma unroll
+        for (int a = 0; a < NACC; ++a) s.acc[a] += v[a];
+      }
+    }
+  }
+  __syncwarp();
+  if (lane == 0) {
+    ws.ihead = (ihead + n) & (kItemQ - 1);
+    ws.icount -= n;
+  }
+  __syncwarp();
+}
+
+// ---------------------------------------------------------------------------------------------------- z-stage
+// Expand the first nb (<= EPW = 32/G) queued exposures of the current tile into subsamples, G = min(n_ss,32) lanes each:
+// pinned subsample time and phase fold (H1, H2), orbit, in-transit test; compacts the in-transit subsamples into
+// the item queue.  Runs basis rounds itself whenever 32 items are waiting.
+template <int MODE, bool NPB1, bool SS1, typename OutT>
+__device__ __noinline__ void expand(const FluxArgs& A, WarpState& ws, int nb) {
+  const int lane = threadIdx.x & 31;
+  const unsigned lt = (1u << lane) - 1u;
+  const int cur = ws.cur;
+  const PvRec& r = ws.pv[cur];
+  const int n_pb = NPB1 ? 1 : A.n_pb;
+  const int n_ss = SS1 ? 1 : A.n_ss;
+  const int G = n_ss < 32 ? n_ss : 32;
+  const int grp = SS1 ? lane : lane / G, g = SS1 ? 0 : lane - grp * G;
+  const bool act = grp < nb;
+  const int qhead = ws.qhead;
+  const uint32_t e = act ? ws.expq[(qhead + grp) & (kExpQ - 1)] : 0u;
+  const double t = act ? __ldg(r.tb + e) : 0.0;
+  const double khat = r.c.khat;
+  const bool slow_div = r.c.flags & PV_SLOWDIV;
+  OutT* ob = (OutT*)r.ob;
+  if (SS1) {
+    bool p = false;
+    double zs = 0.0;
+    if (act) {
+      zs = orbit_z_signed(r.c, fold_phase(t, r.c.t0, r.c.P, r.c.invP, slow_div));
+      p = zs >= 0.0 && zs < 1.0 + khat;
+      if (!p) store_one<NPB1, OutT>(ob + e, A.n_t, n_pb);
+    }
+    const unsigned m = __ballot_sync(0xffffffffu, p);
+    if (p) {
+      const int pos = (ws.ihead + ws.icount + __popc(m & lt)) & (kItemQ - 1);
+      ws.item_z[pos] = zs;
+      ws.item_tag[pos] = (uint16_t)e;
+      ws.item_ring[pos] = (uint8_t)cur;
+    }
+    __syncwarp();
+    if (lane == 0) {
+      ws.icount += __popc(m);
+      ws.qhead = (qhead + nb) & (kExpQ - 1);
+      ws.qcount -= nb;
+    }
+    __syncwarp();
+  } else {
+    const bool multi = n_ss > 32;             // one exposure per round, several sub-rounds of 32 subsamples
+    const unsigned gmask = (G == 32 ? 0xffffffffu : ((1u << G) - 1u)) << (grp * G);
+    const unsigned below = (grp * G >= 32) ? 0xffffffffu : ((1u << (grp * G)) - 1u);   // lanes of earlier groups
+    int sid = -1;
+    for (int s0 = 0; s0 < n_ss; s0 += 32) {
+      const int s = s0 + g;
+      bool p = false;
+      double zs = 0.0;
+      if (act && s < n_ss) {
+        const double ts = __dadd_rn(t, subsample_offset(s, n_ss, A.t_exp));
+        zs = orbit_z_signed(r.c, fold_phase(ts, r.c.t0, r.c.P, r.c.invP, slow_div));
+        p = zs >= 0.0 && zs < 1.0 + khat;
+      }
+      const unsigned m = __ballot_sync(0xffffffffu, p);
+      int nalloc = 0;
+      if (!multi) {
+        const int cnt = __popc(m & gmask);
+        const bool has = act && cnt > 0;
+        const unsigned hm = __ballot_sync(0xffffffffu, has && g == 0);
+        sid = (ws.slot_next + __popc(hm & below)) & (kSlots - 1);
+        nalloc = __popc(hm);
+        if (act && g == 0) {
+          if (has) {
+            Slot& sl = ws.slots[sid];
+            sl.acc[0] = 0; sl.acc[1] = 0; sl.acc[2] = 0;
+            sl.remaining = cnt; sl.e = (uint16_t)e; sl.ring = (uint16_t)cur;
+          } else {
+            store_one<NPB1, OutT>(ob + e, A.n_t, n_pb);
+          }
+        }
+      } else if (m) {
+        if (sid < 0) {
+          sid = ws.slot_next & (kSlots - 1);
+          nalloc = 1;
+          if (lane == 0) {
+            Slot& sl = ws.slots[sid];
+            sl.acc[0] = 0; sl.acc[1] = 0; sl.acc[2] = 0;
+            sl.remaining = kRemBias; sl.e = (uint16_t)e; sl.ring = (uint16_t)cur;
+          }
+          __syncwarp();
+        }
+        if (lane == 0) ws.slots[sid].remaining += __popc(m);
+      }
+      if (p) {
+        const int pos = (ws.ihead + ws.icount + __popc(m & lt)) & (kItemQ - 1);
+        ws.item_z[pos] = zs;
+        ws.item_tag[pos] = (uint16_t)sid;
+      }
+      __syncwarp();
+      if (lane == 0) {
+        ws.icount += __popc(m);
+        ws.slot_next = (ws.slot_next + nalloc) & (kSlots - 1);
+      }
+      __syncwarp();
+      if (multi) while (ws.icount >= 32) basis_round<MODE, NPB1, SS1, OutT>(A, ws, 32);
+    }
+    if (multi) {
+      if (sid < 0) {
+        if (lane == 0) store_one<NPB1, OutT>(ob + e, A.n_t, n_pb);
+      } else if (lane == 0) {
+        Slot& sl = ws.slots[sid];
+        const int rem = sl.remaining - kRemBias;
+        sl.remaining = rem;
+        if (rem == 0) {   // every subsample was already evaluated by the basis rounds in between
+          if (NPB1) finish_exposure<true, OutT>(A, ws, r, e, (double)sl.acc[0] * r.acc_inv, 0.0, 0.0);
+          else finish_exposure<false, OutT>(A, ws, r, e, (double)sl.acc[0] * A.fx_inv, (double)sl.acc[1] * A.fx_inv,
+                                            (double)sl.acc[2] * A.fx_inv);
+        }
+      }
+    }
+    __syncwarp();
+    if (lane == 0) {
+      ws.qhead = (qhead + nb) & (kExpQ - 1);
+      ws.qcount -= nb;
+    }
+    __syncwarp();
+  }
+  while (ws.icount >= 32) basis_round<MODE, NPB1, SS1, OutT>(A, ws, 32);
+}
+
+// Drain the item queue completely (ragged last batch): before a PvRec that live items refer to is overwritten, and at
+// the end of the kernel.
+template <int MODE, bool NPB1, bool SS1, typename OutT>
+__device__ __forceinline__ void drain_items(const FluxArgs& A, WarpState& ws) {
+  while (ws.icount > 0) basis_round<MODE, NPB1, SS1, OutT>(A, ws, min(ws.icount, 32));
+}
+
+// ---------------------------------------------------------------------------------------------------- the kernel
+// MODE 0: exact.  MODE 1: interpolated (exact basis functions for a parameter vector whose k̂ is off the table).
+// V: exposures per lane and load/store in the stream stage (2 = 16-byte ld/st, needs even row lengths/strides and
+// 16-byte aligned bases).  NPB1: single passband.  SS1: n_ss == 1 (no supersample accumulation).
+template <int MODE, int V, bool NPB1, bool SS1, typename OutT>
+__global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const FluxArgs A) {
+  __shared__ WarpState s_ws[kWarpsPerBlock];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  WarpState& ws = s_ws[warp];
+  if (lane == 0) {
+    ws.qhead = 0; ws.qcount = 0; ws.ihead = 0; ws.icount = 0; ws.slot_next = 0; ws.cur = 0;
+  }
+  __syncwarp();
+  const int n_pb = NPB1 ? 1 : A.n_pb;
+  const int n_ss = SS1 ? 1 : A.n_ss;
+  const int EPW = 32 / (n_ss < 32 ? n_ss : 32);
+  constexpr uint32_t kSuper = 32u * kUnroll * V;
+  const int64_t gw = (int64_t)blockIdx.x * kWarpsPerBlock + warp, nw = (int64_t)gridDim.x * kWarpsPerBlock;
+
+  for (int64_t tile = gw; tile < A.n_tiles; tile += nw) {
+    // the PvRec this tile will use must not be referenced by queued subsamples any more
+    const int ring = NPB1 ? ((ws.cur + 1) & (kPvRing - 1)) : 0;
+    if (ws.icount > 0) {
+      bool clash = true;
+      if (NPB1) {
+        const int ih = ws.ihead;
+        const int oldest = SS1 ? (int)ws.item_ring[ih] : (int)ws.slots[ws.item_tag[ih]].ring;
+        clash = (oldest == ring);
+      }
+      if (clash) drain_items<MODE, NPB1, SS1, OutT>(A, ws);
+    }
+    tile_setup<MODE, NPB1, OutT>(A, ws, ring, tile);
+    if (lane == 0) ws.cur = ring;
+    __syncwarp();
+    const PvRec& r = ws.pv[ring];
+    const int chunk = (int)(tile % A.tiles_per_pv);
+    const uint32_t n_e = (uint32_t)min((int64_t)A.tile_len, A.n_t - (int64_t)chunk * A.tile_len);
+    const double* __restrict__ tb = r.tb;
+    OutT* __restrict__ ob = (OutT*)r.ob;
+
+    if (r.c.flags & PV_BAD) {
+      for (int j = 0; j < n_pb; ++j)
+        for (uint32_t e = lane; e < n_e; e += 32) ob[(int64_t)j * A.n_t + e] = (OutT)nan64();
+      continue;
+    }
+    const double w_invP = r.c.invP, w_c0 = r.w_c0, w_half = r.w_half;
+
+    for (uint32_t base = 0; base < n_e; base += kSuper) {
+      unsigned inw = 0;                                          // bit (u*V+v): exposure (u,v) of this lane is in the window
+      if (base + kSuper <= n_e) {                                // warp-uniform
+        double t[kUnroll][V];
+#pragma unroll
+        for (int u = 0; u < kUnroll; ++u) {                      // all loads first: kUnroll independent requests per lane
+          const uint32_t e = base + (u * 32 + lane) * V;
+          if (V == 2) { const double2 tv = __ldg((const double2*)(tb + e)); t[u][0] = tv.x; t[u][V - 1] = tv.y; }
+          else t[u][0] = __ldg(tb + e);
+        }
+#pragma unroll
+        for (int u = 0; u < kUnroll; ++u) {
+          const uint32_t e = base + (u * 32 + lane) * V;
+          unsigned pair = 0;
+#pragma unroll
+          for (int v = 0; v < V; ++v) pair |= in_window2(t[u][v], w_invP, w_c0, w_half) ? (1u << v) : 0u;
+          inw |= pair << (u * V);
+          if (V == 2 && pair == 0) store_one_pair<NPB1, OutT>(ob + e, A.n_t, n_pb);
+          else {
+#pragma unroll
+            for (int v = 0; v < V; ++v) if (!((pair >> v) & 1u)) store_one<NPB1, OutT>(ob + e + v, A.n_t, n_pb);
+          }
+        }
+      } else {
+#pragma unroll
+        for (int u = 0; u < kUnroll; ++u) {
+#pragma unroll
+          for (int v = 0; v < V; ++v) {
+            const uint32_t e = base + (u * 32 + lane) * V + v;
+            if (e < n_e) {
+              if (in_window2(__ldg(tb + e), w_invP, w_c0, w_half)) inw |= 1u << (u * V + v);
+              else store_one<NPB1, OutT>(ob + e, A.n_t, n_pb);
+            }
+          }
+        }
+      }
+      // append the in-window exposures to the exposure ring: warp prefix sum of the per-lane counts
+      if (__reduce_or_sync(0xffffffffu, inw)) {
+        const int cnt = __popc(inw);
+        int incl = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const int up = __shfl_up_sync(0xffffffffu, incl, o);
+          if (lane >= o) incl += up;
+        }
+        const int total = __shfl_sync(0xffffffffu, incl, 31);
+        int pos = ws.qhead + ws.qcount + incl - cnt;
+        while (inw) {
+          const int b = __ffs(inw) - 1;
+          inw &= inw - 1u;
+          ws.expq[pos & (kExpQ - 1)] = (uint16_t)(base + ((b / V) * 32 + lane) * V + (b % V));
+          ++pos;
+        }
+        __syncwarp();
+        if (lane == 0) ws.qcount += total;
+        __syncwarp();
+        while (ws.qcount >= EPW) expand<MODE, NPB1, SS1, OutT>(A, ws, EPW);
+      }
+    }
+    // end of tile: the exposure ring refers to this tile's indices, so it is emptied here (ragged z-round, cheap)
+    while (ws.qcount > 0) expand<MODE, NPB1, SS1, OutT>(A, ws, min(ws.qcount, EPW));
+    if (!NPB1) drain_items<MODE, NPB1, SS1, OutT>(A, ws);   // the coefficient cache belongs to this parameter vector
+  }
+  drain_items<MODE, NPB1, SS1, OutT>(A, ws);
+}
+
+}  // namespace pt

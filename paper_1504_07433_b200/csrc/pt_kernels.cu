@@ -1,312 +1,18 @@
 // pt_kernels.cu — sm_100a kernels and the C ABI of include/pt.h.
 //
-// One fused kernel evaluates the whole hot path for a tile of exposures of one parameter vector:
-//   phase A  every exposure: coalesced time load, cheap phase-window test; exposures that cannot be in transit keep
-//            basis = 0 (flux exactly 1); the others are appended to a block-local queue (warp ballot + one smem atomic)
-//   phase B  dense warps drain the queue: a group of G = min(n_ss,32) lanes owns one queued exposure, each lane
-//            evaluates its subsamples (pinned fold -> orbit -> Mandel–Agol basis functions or table lookup), the group
-//            reduces λe, λd, ηd with a segmented warp shuffle and the head lane stores the means in shared memory
-//   phase C  all threads: per passband linear combine and coalesced (16-byte where aligned) stores
-// The queue is the "binning" that limits divergence: warps in phase B hold only (probably) in-transit samples, and
-// inside/partial lanes differ only in the coefficients they feed to the shared elliptic-integral loop.
+// The fused flux kernel (whole hot path in one persistent launch) lives in pt_flux.cuh; this file holds the orbit-only
+// kernel, the table builder, the FP64 probe and the host side of the C ABI.
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 #include <atomic>
 
 #include "../../include/pt.h"
-#include "pt_basis.cuh"
-#include "pt_orbit.cuh"
+#include "pt_flux.cuh"
 
 namespace pt {
 
-constexpr int kThreads = 256;
-#ifndef PT_MIN_BLOCKS
-#define PT_MIN_BLOCKS 3   // resident blocks per SM the flux kernel is compiled for (register cap 65536/(256*PT_MIN_BLOCKS))
-#endif
-constexpr int kMaxPassbands = 1024;  // 3 doubles of shared memory each
-constexpr int kUnroll = 4;            // 32-exposure groups a warp streams per iteration (independent loads in flight)
-constexpr int kQueue = 512;           // per-warp ring queue: > 2*32*kUnroll + 32 entries, power of two
-
 static std::atomic<int64_t> g_launches{0};
-
-struct FluxArgs {
-  const double* times;
-  int64_t n_t, t_stride_pv;
-  const double* params;
-  int64_t n_pv;
-  int n_pb, n_ss;
-  double t_exp;
-  void* flux;
-  int32_t* status;
-  int blocks_per_pv;
-  int64_t exp_per_block;
-  // interpolation table (mode 1)
-  const void* tb;
-  int tb_dtype, n_k, n_z, n_fn;
-  double k_min, dk, dz, inv_dk, inv_dz;
-};
-
-__device__ __forceinline__ double nan64() { return __longlong_as_double(0x7ff8000000000000LL); }
-
-// Per-block setup: validate the row, mean radius ratio, per-passband combine coefficients, orbit constants + window.
-// coef[3*j + 0..2] = g_j (1-c_j)/N_j, g_j c_j/N_j, g_j u2_j/N_j with g_j = k_j²/k̂².
-__device__ void block_setup(PvConst& c, double* coef, const double* row, int n_pb, int n_ss, double t_exp) {
-  __shared__ int s_ok;
-  if (threadIdx.x == 0) s_ok = 1;
-  __syncthreads();
-  bool ok = true;
-  for (int j = threadIdx.x; j < n_pb; j += blockDim.x) {
-    const double k = row[6 + 3 * j], u1 = row[7 + 3 * j], u2 = row[8 + 3 * j];
-    const double N = 1.0 - u1 / 3.0 - u2 / 6.0;
-    if (!(isfinite(k) && isfinite(u1) && isfinite(u2)) || !(k >= 0.0) || N == 0.0) ok = false;
-  }
-  if (!ok) s_ok = 0;
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    double ksum = 0.0;
-    for (int j = 0; j < n_pb; ++j) ksum += row[6 + 3 * j];   // index order (R9)
-    c.khat = ksum / (double)n_pb;
-    pv_setup_orbit(c, row, s_ok != 0, n_ss, t_exp);
-  }
-  __syncthreads();
-  if (c.flags & PV_BAD) return;
-  const double ik2 = c.khat > 0.0 ? 1.0 / (c.khat * c.khat) : 0.0;
-  for (int j = threadIdx.x; j < n_pb; j += blockDim.x) {
-    const double k = row[6 + 3 * j], u1 = row[7 + 3 * j], u2 = row[8 + 3 * j];
-    const double cj = u1 + 2.0 * u2;
-    const double gN = k * k * ik2 / (1.0 - u1 / 3.0 - u2 / 6.0);
-    coef[3 * j + 0] = gN * (1.0 - cj);
-    coef[3 * j + 1] = gN * cj;
-    coef[3 * j + 2] = gN * u2;
-  }
-  __syncthreads();
-}
-
-// Bilinear lookup of the three functions.  Corner loads go through the read-only path; the table is
-// expected to live in L2.
-template <typename TT>
-__device__ __forceinline__ Basis table_lookup(const FluxArgs& A, int ik, double fk, double z) {
-  const double rz = z / A.dz;
-  int iz = (int)floor(rz);
-  iz = min(max(iz, 0), A.n_z - 2);
-  const double fz = rz - (double)iz;
-  const TT* r0 = (const TT*)A.tb + ((size_t)ik * A.n_z + iz) * A.n_fn;
-  const TT* r1 = r0 + (size_t)A.n_z * A.n_fn;
-  double v[3];
-#pragma unroll
-  for (int f = 0; f < 3; ++f) {
-    const double t00 = (double)__ldg(r0 + f), t01 = (double)__ldg(r0 + A.n_fn + f);
-    const double t10 = (double)__ldg(r1 + f), t11 = (double)__ldg(r1 + A.n_fn + f);
-    const double lo = fma(fz, t01 - t00, t00);
-    const double hi = fma(fz, t11 - t10, t10);
-    v[f] = fma(fk, hi - lo, lo);
-  }
-  Basis b;
-  b.le = v[0]; b.ld = v[1]; b.ed = v[2];
-  return b;
-}
-
-// Per-passband combine and streaming stores of one exposure's fluxes.
-template <bool NPB1, typename OutT>
-__device__ __forceinline__ void store_exposure(OutT* __restrict__ out, int64_t n_t, int n_pb,
-                                               const double* __restrict__ coef, double le, double ld, double ed) {
-  if (NPB1) {
-    __stcs(out, (OutT)(1.0 - fma(coef[2], ed, fma(coef[1], ld, coef[0] * le))));
-  } else {
-    for (int j = 0; j < n_pb; ++j) {
-      const double v = 1.0 - fma(coef[3 * j + 2], ed, fma(coef[3 * j + 1], ld, coef[3 * j] * le));
-      __stcs(out + (int64_t)j * n_t, (OutT)v);
-    }
-  }
-}
-template <bool NPB1, typename OutT>
-__device__ __forceinline__ void store_one(OutT* __restrict__ out, int64_t n_t, int n_pb) {
-  if (NPB1) __stcs(out, (OutT)1.0);
-  else for (int j = 0; j < n_pb; ++j) __stcs(out + (int64_t)j * n_t, (OutT)1.0);
-}
-template <typename OutT> struct Vec2;
-template <> struct Vec2<double> { typedef double2 type; };
-template <> struct Vec2<float> { typedef float2 type; };
-template <bool NPB1, typename OutT>
-__device__ __forceinline__ void store_one_pair(OutT* __restrict__ out, int64_t n_t, int n_pb) {
-  typename Vec2<OutT>::type v;
-  v.x = (OutT)1.0; v.y = (OutT)1.0;
-  if (NPB1) __stcs((typename Vec2<OutT>::type*)out, v);
-  else for (int j = 0; j < n_pb; ++j) __stcs((typename Vec2<OutT>::type*)(out + (int64_t)j * n_t), v);
-}
-
-// MODE 0: exact.  MODE 1: interpolated (falls back to exact for a parameter vector whose k̂ is off the table).
-// V: exposures per lane and load/store (2 = 16-byte ld/st.v2.f64, needs even row lengths and 16-byte aligned bases).
-// NPB1: single passband (one store per exposure, no passband loop).
-//
-// Every warp is autonomous after the per-block setup (no block barrier in the loop): it streams kUnroll*32*V exposures
-// at a time (all loads issued first), stores flux = 1 for those that fail the phase-window test, and keeps the others in
-// a private ring queue; as soon as the queue holds a full batch (EPW = 32/G exposures, G = min(n_ss,32) lanes each) the
-// warp evaluates it with all lanes busy.  Warps of a block take interleaved super-groups, so in-transit work is spread
-// over the block.
-template <int MODE, int V, bool NPB1, typename OutT>
-__global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const FluxArgs A) {
-  extern __shared__ double s_coef[];   // 3 * n_pb
-  __shared__ PvConst c;
-  __shared__ uint32_t s_queue[kThreads / 32][kQueue];
-
-  const int64_t pv = blockIdx.x / A.blocks_per_pv;
-  const int chunk = (int)(blockIdx.x % A.blocks_per_pv);
-  const double* row = A.params + pv * (6 + 3 * (int64_t)A.n_pb);
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int n_pb = NPB1 ? 1 : A.n_pb;
-
-  block_setup(c, s_coef, row, n_pb, A.n_ss, A.t_exp);
-
-  const int64_t e_begin = (int64_t)chunk * A.exp_per_block;
-  const uint32_t n_e = (uint32_t)min((int64_t)A.exp_per_block, A.n_t - e_begin);   // exposures of this block (< 2^31)
-  const double* __restrict__ tb = A.times + pv * A.t_stride_pv + e_begin;
-  OutT* __restrict__ ob = (OutT*)A.flux + pv * n_pb * A.n_t + e_begin;
-  const int flags = c.flags;
-
-  if (flags & PV_BAD) {
-    for (int j = 0; j < n_pb; ++j)
-      for (uint32_t e = tid; e < n_e; e += kThreads) ob[(int64_t)j * A.n_t + e] = (OutT)nan64();
-    if (chunk == 0 && tid == 0 && A.status) {
-      atomicOr(&A.status[0], PT_ST_BAD_PARAM);
-      atomicAdd(&A.status[1], 1);
-    }
-    return;
-  }
-
-  bool use_table = false;
-  int ik = 0;
-  double fk = 0.0;
-  if (MODE == 1) {
-    const double rk = (c.khat - A.k_min) / A.dk;
-    use_table = (c.khat >= A.k_min) && (c.khat <= A.k_min + (A.n_k - 1) * A.dk);
-    ik = min(max((int)floor(rk), 0), A.n_k - 2);
-    fk = rk - (double)ik;
-    if (!use_table && !(flags & PV_NEVER) && chunk == 0 && tid == 0 && A.status) {
-      atomicOr(&A.status[0], PT_ST_K_OUT_OF_TABLE);
-      atomicAdd(&A.status[1], 1);
-    }
-  }
-
-  // lane -> (slot, g): G lanes per queued exposure, EPW exposures per batch
-  const int n_ss = A.n_ss;
-  const int G = n_ss < 32 ? n_ss : 32;
-  const int EPW = 32 / G;
-  const int slot = lane / G, g = lane - slot * G;
-  const double off0 = (n_ss > 1) ? subsample_offset(g, n_ss, A.t_exp) : 0.0;
-  const double inv_nss = 1.0 / (double)n_ss;
-  const double khat = c.khat;
-  const bool slow_div = flags & PV_SLOWDIV;
-  const double w_t0 = c.t0, w_invP = c.invP, w_mid = c.win_mid, w_half = c.win_half;
-  uint32_t* queue = s_queue[warp];
-  int qhead = 0, qcount = 0;   // warp-uniform
-
-  // evaluate the first `nb` queued exposures (nb <= EPW) with G lanes each
-  auto process_batch = [&](int nb) {
-    const bool act = slot < nb;
-    double ale = 0.0, ald = 0.0, aed = 0.0;
-    uint32_t e = 0;
-    if (act) {
-      e = queue[(qhead + slot) & (kQueue - 1)];
-      const double t = __ldg(tb + e);
-      for (int s = g; s < n_ss; s += G) {
-        const double off = (s == g) ? off0 : subsample_offset(s, n_ss, A.t_exp);
-        const double ts = (n_ss > 1) ? __dadd_rn(t, off) : t;
-        const double ph = fold_phase(ts, c.t0, c.P, c.invP, slow_div);
-        const double zs = orbit_z_signed(c, ph);
-        if (zs >= 0.0 && zs < 1.0 + khat) {
-          Basis b;
-          if (MODE == 1 && use_table) {
-            b = (A.tb_dtype == PT_F64) ? table_lookup<double>(A, ik, fk, zs) : table_lookup<float>(A, ik, fk, zs);
-          } else {
-            b = ma_basis(khat, zs);
-          }
-          ale += b.le; ald += b.ld; aed += b.ed;
-        }
-      }
-    }
-    if (G > 1) {   // segmented sum over the G lanes of each exposure (warp-uniform branch, full-warp shuffles)
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const double tle = __shfl_down_sync(0xffffffffu, ale, o);
-        const double tld = __shfl_down_sync(0xffffffffu, ald, o);
-        const double ted = __shfl_down_sync(0xffffffffu, aed, o);
-        if (g + o < G) { ale += tle; ald += tld; aed += ted; }
-      }
-    }
-    if (act && g == 0)
-      store_exposure<NPB1>(ob + e, A.n_t, n_pb, s_coef, ale * inv_nss, ald * inv_nss, aed * inv_nss);
-    qhead = (qhead + nb) & (kQueue - 1);
-    qcount -= nb;
-  };
-
-  // super-groups of kUnroll x 32 lanes x V exposures, interleaved over the warps of the block
-  constexpr int kWarps = kThreads / 32;
-  constexpr uint32_t kSuper = 32u * kUnroll * V;
-  const uint32_t n_super = (n_e + kSuper - 1) / kSuper;
-  const uint32_t n_iter = (n_super + kWarps - 1) / kWarps;   // same trip count for every warp
-  for (uint32_t it = 0; it < n_iter; ++it) {
-    const uint32_t base = (it * kWarps + warp) * kSuper;      // may lie beyond n_e for the last iteration
-    const bool full = base + kSuper <= n_e;                    // warp-uniform
-    double t[kUnroll][V];
-    unsigned inw = 0;                                          // bit (u*V+v): exposure (u,v) of this lane is in the window
-    if (full) {
-#pragma unroll
-      for (int u = 0; u < kUnroll; ++u) {                      // all loads first: kUnroll independent requests per lane
-        const uint32_t e = base + (u * 32 + lane) * V;
-        if (V == 2) { const double2 tv = __ldg((const double2*)(tb + e)); t[u][0] = tv.x; t[u][V - 1] = tv.y; }
-        else t[u][0] = __ldg(tb + e);
-      }
-#pragma unroll
-      for (int u = 0; u < kUnroll; ++u) {
-        const uint32_t e = base + (u * 32 + lane) * V;
-#pragma unroll
-        for (int v = 0; v < V; ++v) inw |= in_window(t[u][v], w_t0, w_invP, w_mid, w_half) ? (1u << (u * V + v)) : 0u;
-        const unsigned pair = (inw >> (u * V)) & (V == 2 ? 3u : 1u);
-        if (V == 2 && pair == 0) store_one_pair<NPB1>(ob + e, A.n_t, n_pb);
-        else {
-#pragma unroll
-          for (int v = 0; v < V; ++v) if (!((pair >> v) & 1u)) store_one<NPB1>(ob + e + v, A.n_t, n_pb);
-        }
-      }
-    } else {
-#pragma unroll
-      for (int u = 0; u < kUnroll; ++u) {
-#pragma unroll
-        for (int v = 0; v < V; ++v) {
-          const uint32_t e = base + (u * 32 + lane) * V + v;
-          if (e < n_e) {
-            if (in_window(__ldg(tb + e), w_t0, w_invP, w_mid, w_half)) inw |= 1u << (u * V + v);
-            else store_one<NPB1>(ob + e, A.n_t, n_pb);
-          }
-        }
-      }
-    }
-    // append the in-window exposures to the ring queue: one ballot per (u,v) slot that has any taker in the warp
-    // (REDUX.OR finds those slots in one instruction; typically 0-2 of the kUnroll*V are non-empty)
-    unsigned slots = __reduce_or_sync(0xffffffffu, inw);
-    if (slots) {
-      const unsigned lt = (1u << lane) - 1u;
-      do {
-        const int uv = __ffs(slots) - 1;
-        slots &= slots - 1u;
-        const bool b = (inw >> uv) & 1u;
-        const unsigned m = __ballot_sync(0xffffffffu, b);
-        if (b) queue[(qhead + qcount + __popc(m & lt)) & (kQueue - 1)] = base + ((uv / V) * 32 + lane) * V + (uv % V);
-        qcount += __popc(m);
-      } while (slots);
-      __syncwarp();
-    }
-    const bool last = (it + 1 == n_iter);
-    if (qcount >= EPW || (last && qcount > 0)) {
-      do {   // full batches; the ragged remainder only after the last group
-        process_batch(min(qcount, EPW));
-      } while (qcount >= EPW || (last && qcount > 0));
-      __syncwarp();
-    }
-  }
-}
 
 // S1-S2 alone: signed projected separation of every subsample.
 __global__ void __launch_bounds__(kThreads) orbit_kernel(const double* __restrict__ times, int64_t n_t,
@@ -386,6 +92,19 @@ static int check_common(const void* times, const void* params, const void* out, 
   return PT_OK;
 }
 
+// Number of SMs of the current device (the persistent grid is sized from it), cached per device.
+static int sm_count() {
+  static std::atomic<int> cached[64];
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 148;
+  int n = cached[dev].load();
+  if (n == 0) {
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+    cached[dev].store(n);
+  }
+  return n;
+}
+
 static int launch_flux(int mode, const pt_table* tb, const double* d_times, int64_t n_t, int64_t t_stride_pv,
                        const double* d_params, int64_t n_pv, int n_pb, int n_ss, double t_exp, int dtype, void* d_flux,
                        int32_t* d_status, cudaStream_t st) {
@@ -400,32 +119,44 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
         !(tb->dz > 0.0) || (tb->dtype != PT_F64 && tb->dtype != PT_F32))
       return PT_ERR_TABLE;
     A.tb = tb->d_data; A.tb_dtype = tb->dtype; A.n_k = tb->n_k; A.n_z = tb->n_z; A.n_fn = tb->n_fn;
-    A.k_min = tb->k_min; A.dk = tb->dk; A.dz = tb->dz; A.inv_dk = 1.0 / tb->dk; A.inv_dz = 1.0 / tb->dz;
+    A.k_min = tb->k_min; A.dk = tb->dk; A.dz = tb->dz;
   }
-  // exposures per block: a multiple of 256 (32 per warp-iteration), at least 2048 when the row is that long, chosen so
-  // that the grid has about 8 blocks per SM
-  const int64_t target_blocks = 148 * 8;
-  int64_t bpp = (target_blocks + n_pv - 1) / n_pv;
-  int64_t epb = (n_t + bpp - 1) / bpp;
-  if (epb < 2048) epb = 2048;
-  epb = (epb + 255) / 256 * 256;
-  if (epb > ((int64_t)1 << 31)) return PT_ERR_SIZE;
-  bpp = (n_t + epb - 1) / epb;
-  if (n_pv * bpp > 0x7fffffff) return PT_ERR_SIZE;
-  A.blocks_per_pv = (int)bpp; A.exp_per_block = epb;
-  const dim3 grid((unsigned)(n_pv * bpp));
-  const size_t smem = (size_t)3 * n_pb * sizeof(double);
+  // persistent grid: PT_MIN_BLOCKS blocks of 8 autonomous warps per SM; tiles of `tile_len` exposures of one parameter
+  // vector are dealt to the warps in strided order, about kTilesPerWarp each so that heavy and light tiles average out
+  const int64_t warps = (int64_t)sm_count() * PT_MIN_BLOCKS * kWarpsPerBlock;
+  constexpr int64_t kTilesPerWarp = 6;
+  const double total = (double)n_pv * (double)n_t;
+  int64_t tl = (int64_t)(total / (double)(warps * kTilesPerWarp));
+  tl = (tl + 255) / 256 * 256;
+  if (tl < 256) tl = 256;
+  if (tl > 16384) tl = 16384;
+  const int64_t tpp = (n_t + tl - 1) / tl;
+  if (tpp > 0x7fffffff || (double)tpp * (double)n_pv > 9.0e18) return PT_ERR_SIZE;
+  A.tile_len = (int)tl; A.tiles_per_pv = (int)tpp; A.n_tiles = n_pv * tpp;
+  int lg = 0;
+  while (((int64_t)1 << lg) < (int64_t)n_ss) ++lg;
+  A.fx_bits = 61 - lg;
+  A.fx_scale = ldexp(1.0, A.fx_bits);
+  A.fx_inv = 1.0 / (A.fx_scale * (double)n_ss);
+  int64_t blocks = (A.n_tiles + kWarpsPerBlock - 1) / kWarpsPerBlock;
+  if (blocks > warps / kWarpsPerBlock) blocks = warps / kWarpsPerBlock;
+  const dim3 grid((unsigned)blocks);
   // 16-byte loads/stores need even row lengths/strides and 16-byte aligned bases
   const bool v2 = (n_t % 2 == 0) && (t_stride_pv % 2 == 0) && (reinterpret_cast<uintptr_t>(d_times) % 16 == 0) &&
                   (reinterpret_cast<uintptr_t>(d_flux) % 16 == 0);
-  const bool p1 = (n_pb == 1);
-#define PT_LAUNCH(M, VV, P, T) flux_kernel<M, VV, P, T><<<grid, kThreads, smem, st>>>(A)
+  const bool p1 = (n_pb == 1), s1 = (n_ss == 1);
+#define PT_LAUNCH(M, VV, P, S, T) flux_kernel<M, VV, P, S, T><<<grid, kThreads, 0, st>>>(A)
+#define PT_LAUNCH_S(M, VV, P, T)                             \
+  do {                                                       \
+    if (s1) PT_LAUNCH(M, VV, P, true, T);                    \
+    else PT_LAUNCH(M, VV, P, false, T);                      \
+  } while (0)
 #define PT_LAUNCH_T(M, T)                                    \
   do {                                                       \
-    if (v2 && p1) PT_LAUNCH(M, 2, true, T);                  \
-    else if (v2) PT_LAUNCH(M, 2, false, T);                  \
-    else if (p1) PT_LAUNCH(M, 1, true, T);                   \
-    else PT_LAUNCH(M, 1, false, T);                          \
+    if (v2 && p1) PT_LAUNCH_S(M, 2, true, T);                \
+    else if (v2) PT_LAUNCH_S(M, 2, false, T);                \
+    else if (p1) PT_LAUNCH_S(M, 1, true, T);                 \
+    else PT_LAUNCH_S(M, 1, false, T);                        \
   } while (0)
   if (mode == 0) {
     if (dtype == PT_F64) PT_LAUNCH_T(0, double); else PT_LAUNCH_T(0, float);
@@ -433,6 +164,7 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
     if (dtype == PT_F64) PT_LAUNCH_T(1, double); else PT_LAUNCH_T(1, float);
   }
 #undef PT_LAUNCH_T
+#undef PT_LAUNCH_S
 #undef PT_LAUNCH
   g_launches.fetch_add(1);
   return cudaGetLastError() == cudaSuccess ? PT_OK : PT_ERR_CUDA;
