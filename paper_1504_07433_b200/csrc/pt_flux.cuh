@@ -44,6 +44,9 @@ constexpr int kPvRing = 4;      // parameter-vector records a warp keeps alive (
 constexpr int kCoefCache = 32;  // passbands whose combine coefficients are cached per warp (multi-passband path)
 constexpr int kMaxTileLen = 32768;
 constexpr int kRemBias = 1 << 24;
+#ifndef PT_EXPAND_INLINE
+#define PT_EXPAND_INLINE __forceinline__
+#endif
 
 struct FluxArgs {
   const double* times;
@@ -58,10 +61,12 @@ struct FluxArgs {
   int tile_len;            // exposures per tile (multiple of 256, <= kMaxTileLen)
   int tiles_per_pv;
   int64_t n_tiles;
+  unsigned long long* sched;   // [0] next tile to hand out (beyond the first one per warp), [1] warps that have finished
   // supersample accumulation (fixed point)
   int fx_bits;             // 61 - ceil(log2 n_ss): a sum of n_ss values below 2^eb fits an int64 at scale 2^(fx_bits-eb)
   double fx_scale;         // 2^fx_bits (basis values are <= 1)
   double fx_inv;           // 1 / (fx_scale * n_ss)
+  double inv_nss;          // 1 / n_ss
   // interpolation table (mode 1)
   const void* tb;
   int tb_dtype, n_k, n_z, n_fn;
@@ -200,21 +205,21 @@ __device__ __noinline__ void tile_setup(const FluxArgs& A, WarpState& ws, int ri
   const int n_pb = NPB1 ? 1 : A.n_pb;
   const double* row = A.params + pv * (6 + 3 * (int64_t)n_pb);
   bool ok = true;
-  double ksum = 0.0;
+  double ksum = 0.0, N0 = 1.0;
   for (int j = 0; j < n_pb; ++j) {
     const double k = __ldg(row + 6 + 3 * j), u1 = __ldg(row + 7 + 3 * j), u2 = __ldg(row + 8 + 3 * j);
     const double N = 1.0 - u1 / 3.0 - u2 / 6.0;
     if (!(isfinite(k) && isfinite(u1) && isfinite(u2)) || !(k >= 0.0) || N == 0.0) ok = false;
     ksum += k;
+    if (j == 0) N0 = N;
   }
-  const double khat = ksum / (double)n_pb;
-  PvConst c;
+  const double khat = NPB1 ? ksum : ksum / (double)n_pb;
+  PvConst& c = r.c;          // all lanes store the same values
   c.khat = khat;
   pv_setup_orbit(c, row, ok, A.n_ss, A.t_exp);
   const int64_t e0 = (int64_t)chunk * A.tile_len;
-  const double ik2 = khat > 0.0 ? 1.0 / (khat * khat) : 0.0;
+  const double ik2 = khat > 1.0e-150 ? rcp_fast(khat * khat) : (khat > 0.0 ? 1.0 / (khat * khat) : 0.0);
   if (lane == 0) {
-    r.c = c;
     r.tb = A.times + pv * A.t_stride_pv + e0;
     r.ob = (char*)A.flux + ((pv * n_pb) * A.n_t + e0) * (int64_t)sizeof(OutT);
     r.row = row;
@@ -230,19 +235,18 @@ __device__ __noinline__ void tile_setup(const FluxArgs& A, WarpState& ws, int ri
     return;
   }
   if (NPB1) {
-    const double k = __ldg(row + 6), u1 = __ldg(row + 7), u2 = __ldg(row + 8);
+    const double u1 = __ldg(row + 7), u2 = __ldg(row + 8);
     const double cj = u1 + 2.0 * u2;
-    const double gN = k * k * ik2 / (1.0 - u1 / 3.0 - u2 / 6.0);
+    const double gN = 1.0 / N0;                           // k²/k̂² = 1 for a single passband
     const double c0 = gN * (1.0 - cj), c1 = gN * cj, c2 = gN * u2;
     // fixed-point scale of the combined decrement c0 λe + c1 λd + c2 ηd (each basis value <= 1): 2^eb > |c0|+|c1|+|c2|
     const double B = fabs(c0) + fabs(c1) + fabs(c2);
     int eb = (int)((__double_as_longlong(B) >> 52) & 0x7ff) - 1022;
     if (!(B > 0.0) || !isfinite(B)) eb = 0;
-    const double sc = pow2i(A.fx_bits - eb);
     if (lane == 0) {
       r.coef[0] = c0; r.coef[1] = c1; r.coef[2] = c2;
-      r.acc_scale = sc;
-      r.acc_inv = 1.0 / (sc * (double)A.n_ss);
+      r.acc_scale = pow2i(A.fx_bits - eb);
+      r.acc_inv = pow2i(eb - A.fx_bits) * A.inv_nss;
     }
   } else {
     for (int j = lane; j < n_pb && j < kCoefCache; j += 32) {
@@ -374,8 +378,15 @@ __device__ __noinline__ void basis_round(const FluxArgs& A, WarpState& ws, int n
 // Expand the first nb (<= EPW = 32/G) queued exposures of the current tile into subsamples, G = min(n_ss,32) lanes each:
 // pinned subsample time and phase fold (H1, H2), orbit, in-transit test; compacts the in-transit subsamples into
 // the item queue.  Runs basis rounds itself whenever 32 items are waiting.
+// Per-lane constants of the z-stage, computed once per kernel: group (exposure) and subsample index of the lane, and the
+// pinned subsample offset (H2) when one round covers all subsamples.
+struct LaneCtx {
+  int grp, g;
+  double off0;
+};
+
 template <int MODE, bool NPB1, bool SS1, typename OutT>
-__device__ __noinline__ void expand(const FluxArgs& A, WarpState& ws, int nb) {
+__device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, const LaneCtx& L, int nb) {
   const int lane = threadIdx.x & 31;
   const unsigned lt = (1u << lane) - 1u;
   const int cur = ws.cur;
@@ -383,7 +394,7 @@ __device__ __noinline__ void expand(const FluxArgs& A, WarpState& ws, int nb) {
   const int n_pb = NPB1 ? 1 : A.n_pb;
   const int n_ss = SS1 ? 1 : A.n_ss;
   const int G = n_ss < 32 ? n_ss : 32;
-  const int grp = SS1 ? lane : lane / G, g = SS1 ? 0 : lane - grp * G;
+  const int grp = L.grp, g = L.g;
   const bool act = grp < nb;
   const int qhead = ws.qhead;
   const uint32_t e = act ? ws.expq[(qhead + grp) & (kExpQ - 1)] : 0u;
@@ -423,7 +434,7 @@ __device__ __noinline__ void expand(const FluxArgs& A, WarpState& ws, int nb) {
       bool p = false;
       double zs = 0.0;
       if (act && s < n_ss) {
-        const double ts = __dadd_rn(t, subsample_offset(s, n_ss, A.t_exp));
+        const double ts = __dadd_rn(t, multi ? subsample_offset(s, n_ss, A.t_exp) : L.off0);
         zs = orbit_z_signed(r.c, fold_phase(ts, r.c.t0, r.c.P, r.c.invP, slow_div));
         p = zs >= 0.0 && zs < 1.0 + khat;
       }
@@ -506,7 +517,7 @@ __device__ __forceinline__ void drain_items(const FluxArgs& A, WarpState& ws) {
 // V: exposures per lane and load/store in the stream stage (2 = 16-byte ld/st, needs even row lengths/strides and
 // 16-byte aligned bases).  NPB1: single passband.  SS1: n_ss == 1 (no supersample accumulation).
 template <int MODE, int V, bool NPB1, bool SS1, typename OutT>
-__global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const FluxArgs A) {
+__global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __grid_constant__ FluxArgs A) {
   __shared__ WarpState s_ws[kWarpsPerBlock];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   WarpState& ws = s_ws[warp];
@@ -518,9 +529,22 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const Flu
   const int n_ss = SS1 ? 1 : A.n_ss;
   const int EPW = 32 / (n_ss < 32 ? n_ss : 32);
   constexpr uint32_t kSuper = 32u * kUnroll * V;
+  LaneCtx L;
+  {
+    const int G = n_ss < 32 ? n_ss : 32;
+    L.grp = lane / G;
+    L.g = lane - L.grp * G;
+    L.off0 = (n_ss > 1 && n_ss <= 32) ? subsample_offset(L.g, n_ss, A.t_exp) : 0.0;
+  }
   const int64_t gw = (int64_t)blockIdx.x * kWarpsPerBlock + warp, nw = (int64_t)gridDim.x * kWarpsPerBlock;
 
-  for (int64_t tile = gw; tile < A.n_tiles; tile += nw) {
+  // Tiles are dealt dynamically: a warp starts with tile `gw` and fetches every further one from a global counter (the
+  // fetch is issued before the current tile is processed, so its latency is hidden).  The last warp to finish resets the
+  // counter pair for the next launch that uses this scheduler slot.
+  int64_t tile = gw;
+  while (tile < A.n_tiles) {
+    unsigned long long fetched = 0;
+    if (lane == 0) fetched = atomicAdd(A.sched, 1ULL);
     // the PvRec this tile will use must not be referenced by queued subsamples any more
     const int ring = NPB1 ? ((ws.cur + 1) & (kPvRing - 1)) : 0;
     if (ws.icount > 0) {
@@ -544,6 +568,7 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const Flu
     if (r.c.flags & PV_BAD) {
       for (int j = 0; j < n_pb; ++j)
         for (uint32_t e = lane; e < n_e; e += 32) ob[(int64_t)j * A.n_t + e] = (OutT)nan64();
+      tile = nw + (int64_t)__shfl_sync(0xffffffffu, fetched, 0);
       continue;
     }
     const double w_invP = r.c.invP, w_c0 = r.w_c0, w_half = r.w_half;
@@ -571,16 +596,13 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const Flu
             for (int v = 0; v < V; ++v) if (!((pair >> v) & 1u)) store_one<NPB1, OutT>(ob + e + v, A.n_t, n_pb);
           }
         }
-      } else {
-#pragma unroll
-        for (int u = 0; u < kUnroll; ++u) {
-#pragma unroll
-          for (int v = 0; v < V; ++v) {
-            const uint32_t e = base + (u * 32 + lane) * V + v;
-            if (e < n_e) {
-              if (in_window2(__ldg(tb + e), w_invP, w_c0, w_half)) inw |= 1u << (u * V + v);
-              else store_one<NPB1, OutT>(ob + e, A.n_t, n_pb);
-            }
+      } else {                                                   // ragged end of the tile: rolled, one exposure at a time
+#pragma unroll 1
+        for (int uv = 0; uv < kUnroll * V; ++uv) {
+          const uint32_t e = base + ((uv / V) * 32 + lane) * V + (uv % V);
+          if (e < n_e) {
+            if (in_window2(__ldg(tb + e), w_invP, w_c0, w_half)) inw |= 1u << uv;
+            else store_one<NPB1, OutT>(ob + e, A.n_t, n_pb);
           }
         }
       }
@@ -604,14 +626,22 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const Flu
         __syncwarp();
         if (lane == 0) ws.qcount += total;
         __syncwarp();
-        while (ws.qcount >= EPW) expand<MODE, NPB1, SS1, OutT>(A, ws, EPW);
       }
+      // full z-rounds; at the end of the tile the exposure ring is emptied (it holds this tile's indices), ragged
+      const int keep = (base + kSuper >= n_e) ? 1 : EPW;
+      while (ws.qcount >= keep) expand<MODE, NPB1, SS1, OutT>(A, ws, L, min(ws.qcount, EPW));
     }
-    // end of tile: the exposure ring refers to this tile's indices, so it is emptied here (ragged z-round, cheap)
-    while (ws.qcount > 0) expand<MODE, NPB1, SS1, OutT>(A, ws, min(ws.qcount, EPW));
     if (!NPB1) drain_items<MODE, NPB1, SS1, OutT>(A, ws);   // the coefficient cache belongs to this parameter vector
+    tile = nw + (int64_t)__shfl_sync(0xffffffffu, fetched, 0);
   }
   drain_items<MODE, NPB1, SS1, OutT>(A, ws);
+  if (lane == 0) {
+    const unsigned long long done = atomicAdd(A.sched + 1, 1ULL);
+    if (done == (unsigned long long)nw - 1ULL) {   // every warp has taken its last ticket: nobody reads the pair any more
+      A.sched[0] = 0ULL;
+      A.sched[1] = 0ULL;
+    }
+  }
 }
 
 }  // namespace pt

@@ -14,6 +14,27 @@ namespace pt {
 
 static std::atomic<int64_t> g_launches{0};
 
+// Scheduler slots of the flux kernel (tile counter + finished-warp counter each).  A launch takes the next slot in a ring;
+// the kernel leaves its slot zeroed when it ends, so a slot is clean again long before the ring comes back to it (that
+// would need kSchedSlots launches in flight at once).  This is the only state the library keeps on the device.
+constexpr int kSchedSlots = 4096;
+__device__ unsigned long long g_sched[kSchedSlots][2];
+static std::atomic<uint64_t> g_sched_seq{0};
+
+static unsigned long long* sched_slot() {
+  static std::atomic<unsigned long long*> base[64];
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+  unsigned long long* b = base[dev].load();
+  if (!b) {
+    void* p = nullptr;
+    if (cudaGetSymbolAddress(&p, g_sched) != cudaSuccess) return nullptr;
+    b = (unsigned long long*)p;
+    base[dev].store(b);
+  }
+  return b + 2 * (g_sched_seq.fetch_add(1) % kSchedSlots);
+}
+
 // S1-S2 alone: signed projected separation of every subsample.
 __global__ void __launch_bounds__(kThreads) orbit_kernel(const double* __restrict__ times, int64_t n_t,
                                                          int64_t t_stride_pv, const double* __restrict__ params,
@@ -124,7 +145,7 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   // persistent grid: PT_MIN_BLOCKS blocks of 8 autonomous warps per SM; tiles of `tile_len` exposures of one parameter
   // vector are dealt to the warps in strided order, about kTilesPerWarp each so that heavy and light tiles average out
   const int64_t warps = (int64_t)sm_count() * PT_MIN_BLOCKS * kWarpsPerBlock;
-  constexpr int64_t kTilesPerWarp = 6;
+  constexpr int64_t kTilesPerWarp = 8;
   const double total = (double)n_pv * (double)n_t;
   int64_t tl = (int64_t)(total / (double)(warps * kTilesPerWarp));
   tl = (tl + 255) / 256 * 256;
@@ -138,9 +159,12 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   A.fx_bits = 61 - lg;
   A.fx_scale = ldexp(1.0, A.fx_bits);
   A.fx_inv = 1.0 / (A.fx_scale * (double)n_ss);
+  A.inv_nss = 1.0 / (double)n_ss;
   int64_t blocks = (A.n_tiles + kWarpsPerBlock - 1) / kWarpsPerBlock;
   if (blocks > warps / kWarpsPerBlock) blocks = warps / kWarpsPerBlock;
   const dim3 grid((unsigned)blocks);
+  A.sched = sched_slot();
+  if (!A.sched) return PT_ERR_CUDA;
   // 16-byte loads/stores need even row lengths/strides and 16-byte aligned bases
   const bool v2 = (n_t % 2 == 0) && (t_stride_pv % 2 == 0) && (reinterpret_cast<uintptr_t>(d_times) % 16 == 0) &&
                   (reinterpret_cast<uintptr_t>(d_flux) % 16 == 0);

@@ -129,7 +129,7 @@ __device__ inline double mean_anomaly_of_true(double f, double e) {
 
 // Validate a parameter row and fill the orbit part of PvConst (khat is set by the caller beforehand).
 // `row` = [t0, P, a/R*, i, e, w, ...]; half_exp_phase = half the exposure in cycles (0 when n_ss == 1).
-__device__ inline void pv_setup_orbit(PvConst& c, const double* row, bool row_ok, int n_ss, double t_exp) {
+__device__ __forceinline__ void pv_setup_orbit(PvConst& c, const double* row, bool row_ok, int n_ss, double t_exp) {
   const double t0 = row[0], P = row[1], a = row[2], inc = row[3], e = row[4], w = row[5];
   int flags = 0;
   if (!row_ok || !(isfinite(t0) && isfinite(P) && isfinite(a) && isfinite(inc) && isfinite(e) && isfinite(w)) ||
@@ -139,7 +139,10 @@ __device__ inline void pv_setup_orbit(PvConst& c, const double* row, bool row_ok
   }
   c.t0 = t0; c.P = P; c.invP = __drcp_rn(P); c.a = a; c.e = e;
   if ((__double_as_longlong(P) & 0x000fffffffffffffLL) == 0x000fffffffffffffLL) flags |= PV_SLOWDIV;
-  c.cosi = cos(inc);
+  // cos i, sin i: the lean kernel for ordinary inclinations, the library for anything else
+  double sini;
+  if (fabs(inc) <= 1.0e3) sincos_bounded(inc, &sini, &c.cosi);
+  else sincos(inc, &sini, &c.cosi);
   const double k = c.khat;
   const double margin = 1.0e-7;   // cycles; the cheap fold differs from the pinned one by < 2.3e-16 |x| <= 2.3e-8
   double lo, hi;
@@ -153,7 +156,7 @@ __device__ inline void pv_setup_orbit(PvConst& c, const double* row, bool row_ok
     const double S = (r * r - ci2) / si2 + 1.0e-12;   // sin²φ below this value; si2 == 0 gives ±inf/NaN (handled)
     if (S <= 0.0) { flags |= PV_NEVER; hi = 0.0; }
     else if (!(S < 1.0)) hi = 0.25;
-    else hi = fmin(0.25, asin(sqrt(S)) * (1.0 / kTwoPi));
+    else hi = fmin(0.25, atan2_pos(sqrt_fast(S), sqrt_fast(1.0 - S)) * kC[C_HALF_INVPI]);   // asin(sqrt S) / 2π
     hi = hi * (1.0 + 1.0e-9) + margin;
     lo = -hi;
   } else {
