@@ -156,10 +156,35 @@ __device__ __forceinline__ void finish_exposure(const FluxArgs& A, const WarpSta
   }
 }
 
-// Bilinear lookup of the three functions.  Corner loads go through the read-only path; the table is
-// expected to live in L2.
+// Table loads carry an L2 evict_last policy: the (k,z) table (60-160 MB) is re-read by every parameter vector while
+// gigabytes of write-once flux stream through the same L2 (those go out with evict-first stores).
+__device__ __forceinline__ unsigned long long l2_keep_policy() {
+  unsigned long long pol;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+__device__ __forceinline__ float ldg_keep(const float* p, unsigned long long pol) {
+  float v;
+  asm volatile("ld.global.nc.L2::cache_hint.f32 %0, [%1], %2;" : "=f"(v) : "l"(p), "l"(pol));
+  return v;
+}
+__device__ __forceinline__ double ldg_keep(const double* p, unsigned long long pol) {
+  double v;
+  asm volatile("ld.global.nc.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(p), "l"(pol));
+  return v;
+}
+__device__ __forceinline__ float4 ldg_keep4(const float* p, unsigned long long pol) {
+  float4 v;
+  asm volatile("ld.global.nc.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;"
+               : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p), "l"(pol));
+  return v;
+}
+
+// Bilinear lookup of the three functions: lo = t00 + fz (t01 - t00), hi = t10 + fz (t11 - t10),
+// v = lo + fk (hi - lo).  A padded fp32 table ([k][z][4], 16-byte nodes) is read with one 16-byte load per corner.
 template <typename TT>
 __device__ __forceinline__ Basis table_lookup(const FluxArgs& A, int ik, double fk, double z) {
+  const unsigned long long pol = l2_keep_policy();
   const double rz = z / A.dz;
   int iz = (int)floor(rz);
   iz = min(max(iz, 0), A.n_z - 2);
@@ -167,13 +192,26 @@ __device__ __forceinline__ Basis table_lookup(const FluxArgs& A, int ik, double 
   const TT* r0 = (const TT*)A.tb + ((size_t)ik * A.n_z + iz) * A.n_fn;
   const TT* r1 = r0 + (size_t)A.n_z * A.n_fn;
   double v[3];
+  if (sizeof(TT) == 4 && A.n_fn == 4 && (reinterpret_cast<uintptr_t>(A.tb) & 15) == 0) {
+    const float4 c00 = ldg_keep4((const float*)r0, pol), c01 = ldg_keep4((const float*)r0 + 4, pol);
+    const float4 c10 = ldg_keep4((const float*)r1, pol), c11 = ldg_keep4((const float*)r1 + 4, pol);
+    const double t00[3] = {(double)c00.x, (double)c00.y, (double)c00.z}, t01[3] = {(double)c01.x, (double)c01.y, (double)c01.z};
+    const double t10[3] = {(double)c10.x, (double)c10.y, (double)c10.z}, t11[3] = {(double)c11.x, (double)c11.y, (double)c11.z};
 #pragma unroll
-  for (int f = 0; f < 3; ++f) {
-    const double t00 = (double)__ldg(r0 + f), t01 = (double)__ldg(r0 + A.n_fn + f);
-    const double t10 = (double)__ldg(r1 + f), t11 = (double)__ldg(r1 + A.n_fn + f);
-    const double lo = fma(fz, t01 - t00, t00);
-    const double hi = fma(fz, t11 - t10, t10);
-    v[f] = fma(fk, hi - lo, lo);
+    for (int f = 0; f < 3; ++f) {
+      const double lo = fma(fz, t01[f] - t00[f], t00[f]);
+      const double hi = fma(fz, t11[f] - t10[f], t10[f]);
+      v[f] = fma(fk, hi - lo, lo);
+    }
+  } else {
+#pragma unroll
+    for (int f = 0; f < 3; ++f) {
+      const double t00 = (double)ldg_keep(r0 + f, pol), t01 = (double)ldg_keep(r0 + A.n_fn + f, pol);
+      const double t10 = (double)ldg_keep(r1 + f, pol), t11 = (double)ldg_keep(r1 + A.n_fn + f, pol);
+      const double lo = fma(fz, t01 - t00, t00);
+      const double hi = fma(fz, t11 - t10, t10);
+      v[f] = fma(fk, hi - lo, lo);
+    }
   }
   Basis b;
   b.le = v[0]; b.ld = v[1]; b.ed = v[2];
@@ -297,8 +335,11 @@ __device__ __forceinline__ bool in_window2(double t, double invP, double c0, dou
 
 // ---------------------------------------------------------------------------------------------------- basis stage
 // Evaluate the first n (<= 32) queued subsamples, one per lane.
+#ifndef PT_BASIS_INLINE
+#define PT_BASIS_INLINE __forceinline__
+#endif
 template <int MODE, bool NPB1, bool SS1, typename OutT>
-__device__ __noinline__ void basis_round(const FluxArgs& A, WarpState& ws, int n) {
+__device__ PT_BASIS_INLINE void basis_round(const FluxArgs& A, WarpState& ws, int n) {
   const int lane = threadIdx.x & 31;
   const bool act = lane < n;
   const int ihead = ws.ihead;
@@ -403,27 +444,25 @@ __device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, const 
   const bool slow_div = r.c.flags & PV_SLOWDIV;
   OutT* ob = (OutT*)r.ob;
   if (SS1) {
-    bool p = false;
-    double zs = 0.0;
+    // n_ss == 1: an exposure in the window is almost always in transit, so a second compaction would buy nothing; the
+    // basis functions are evaluated right here, one exposure per lane, and the item queue stays empty.
     if (act) {
-      zs = orbit_z_signed(r.c, fold_phase(t, r.c.t0, r.c.P, r.c.invP, slow_div));
-      p = zs >= 0.0 && zs < 1.0 + khat;
-      if (!p) store_one<NPB1, OutT>(ob + e, A.n_t, n_pb);
-    }
-    const unsigned m = __ballot_sync(0xffffffffu, p);
-    if (p) {
-      const int pos = (ws.ihead + ws.icount + __popc(m & lt)) & (kItemQ - 1);
-      ws.item_z[pos] = zs;
-      ws.item_tag[pos] = (uint16_t)e;
-      ws.item_ring[pos] = (uint8_t)cur;
+      const double zs = orbit_z_signed(r.c, fold_phase(t, r.c.t0, r.c.P, r.c.invP, slow_div));
+      if (zs >= 0.0 && zs < 1.0 + khat) {
+        const Basis b = eval_basis<MODE>(A, r, zs);
+        if (NPB1) finish_exposure<true, OutT>(A, ws, r, e, fma(r.coef[2], b.ed, fma(r.coef[1], b.ld, r.coef[0] * b.le)), 0.0, 0.0);
+        else finish_exposure<false, OutT>(A, ws, r, e, b.le, b.ld, b.ed);
+      } else {
+        store_one<NPB1, OutT>(ob + e, A.n_t, n_pb);
+      }
     }
     __syncwarp();
     if (lane == 0) {
-      ws.icount += __popc(m);
       ws.qhead = (qhead + nb) & (kExpQ - 1);
       ws.qcount -= nb;
     }
     __syncwarp();
+    return;
   } else {
     const bool multi = n_ss > 32;             // one exposure per round, several sub-rounds of 32 subsamples
     const unsigned gmask = (G == 32 ? 0xffffffffu : ((1u << G) - 1u)) << (grp * G);
@@ -502,13 +541,14 @@ __device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, const 
     }
     __syncwarp();
   }
-  while (ws.icount >= 32) basis_round<MODE, NPB1, SS1, OutT>(A, ws, 32);
+  if (!SS1) while (ws.icount >= 32) basis_round<MODE, NPB1, SS1, OutT>(A, ws, 32);
 }
 
 // Drain the item queue completely (ragged last batch): before a PvRec that live items refer to is overwritten, and at
 // the end of the kernel.
 template <int MODE, bool NPB1, bool SS1, typename OutT>
 __device__ __forceinline__ void drain_items(const FluxArgs& A, WarpState& ws) {
+  if (SS1) return;   // the n_ss == 1 path never queues items
   while (ws.icount > 0) basis_round<MODE, NPB1, SS1, OutT>(A, ws, min(ws.icount, 32));
 }
 
@@ -547,7 +587,7 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
     if (lane == 0) fetched = atomicAdd(A.sched, 1ULL);
     // the PvRec this tile will use must not be referenced by queued subsamples any more
     const int ring = NPB1 ? ((ws.cur + 1) & (kPvRing - 1)) : 0;
-    if (ws.icount > 0) {
+    if (!SS1 && ws.icount > 0) {
       bool clash = true;
       if (NPB1) {
         const int ih = ws.ihead;
@@ -577,6 +617,11 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
       unsigned inw = 0;                                          // bit (u*V+v): exposure (u,v) of this lane is in the window
       if (base + kSuper <= n_e) {                                // warp-uniform
         double t[kUnroll][V];
+        if (base + 2 * kSuper <= n_e) {                          // next super-group's times -> L1 while this one is processed
+#pragma unroll
+          for (int u = 0; u < kUnroll; ++u)
+            asm volatile("prefetch.global.L1 [%0];" ::"l"(tb + base + kSuper + (u * 32 + lane) * V));
+        }
 #pragma unroll
         for (int u = 0; u < kUnroll; ++u) {                      // all loads first: kUnroll independent requests per lane
           const uint32_t e = base + (u * 32 + lane) * V;
