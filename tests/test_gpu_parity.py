@@ -301,3 +301,67 @@ def test_config5_full_size_sampled(pt, oracle):
     err = np.abs(f[rows] - ora_exact(oracle, ws))
     assert err.max() <= TOL64, err.max()
     assert f.max() <= 1.0 + 1e-14 and f.min() >= -1e-14
+
+
+# ------------------------------------------------------------------------------------------- pipeline mechanics
+def test_bitwise_reproducible_across_launches(pt):
+    """Tiles are dealt to warps dynamically, so the split of an exposure's subsamples over basis rounds differs from
+    launch to launch; the fixed-point supersample sum makes the flux independent of it."""
+    w = inputs.config2(n_pv=16, n_t=20000)
+    t, p = dev(w.times), dev(w.params)
+    ref = pt.pt_ma_quad_exact(t, p, 1, w.n_ss, w.t_exp).clone()
+    for n_ss in (w.n_ss, 7, 33):
+        ref = pt.pt_ma_quad_exact(t, p, 1, n_ss, w.t_exp).clone()
+        for _ in range(5):
+            again = pt.pt_ma_quad_exact(t, p, 1, n_ss, w.t_exp)
+            assert torch.equal(ref.view(torch.int64), again.view(torch.int64))
+
+
+@pytest.mark.parametrize("n_pv,n_t,n_ss,n_pb", [(3000, 7, 4, 1), (3000, 5, 1, 1), (700, 33, 1, 3), (300, 61, 5, 2), (257, 1, 1, 1)])
+def test_many_short_rows(pt, oracle, n_pv, n_t, n_ss, n_pb):
+    """More parameter vectors than warps, rows far shorter than a tile: every tile is ragged and queues cross tiles."""
+    w = inputs.config3(n_pv=n_pv, n_pb=n_pb, n_t=n_t)
+    w.n_ss, w.t_exp = n_ss, 0.004
+    assert np.abs(gpu_exact(pt, w) - ora_exact(oracle, w)).max() <= TOL64
+
+
+def test_long_exposure_many_subsamples(pt, oracle):
+    """n_ss > 32: an exposure is expanded in several sub-rounds with basis rounds in between; exposures that are only
+    partly in transit and exposures whose subsamples all miss the star sit next to each other."""
+    w = inputs.config2(n_pv=6, n_t=1500)
+    for n_ss, t_exp in ((97, 0.08), (64, 0.02), (200, 0.3)):
+        w.n_ss, w.t_exp = n_ss, t_exp
+        f, r = gpu_exact(pt, w), ora_exact(oracle, w)
+        assert np.abs(f - r).max() <= TOL64
+        assert np.array_equal(f == 1.0, r == 1.0)
+
+
+def test_scheduler_slots_are_reused_cleanly(pt, oracle):
+    """More launches than the library has scheduler slots: each launch must leave its slot zeroed."""
+    w = inputs.config2(n_pv=2, n_t=700)
+    t, p = dev(w.times), dev(w.params)
+    out = torch.empty((2, 1, 700), dtype=torch.float64, device="cuda")
+    for _ in range(4096 + 300):
+        pt.pt_ma_quad_exact(t, p, 1, w.n_ss, w.t_exp, out=out)
+    torch.cuda.synchronize()
+    assert np.abs(out.cpu().numpy() - ora_exact(oracle, w)).max() <= TOL64
+
+
+def test_concurrent_streams(pt, oracle):
+    """Launches on two streams overlap on the device; each has its own scheduler slot."""
+    wa, wb = inputs.config2(n_pv=24, n_t=30000), inputs.config5(oz64(oracle), n_pv=256, n_t=1024)
+    ta, pa, tb_, pb = dev(wa.times), dev(wa.params), dev(wb.times), dev(wb.params)
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    outs = []
+    for _ in range(4):
+        with torch.cuda.stream(sa):
+            fa = pt.pt_ma_quad_exact(ta, pa, 1, wa.n_ss, wa.t_exp)
+        with torch.cuda.stream(sb):
+            fb = pt.pt_ma_quad_exact(tb_, pb)
+        outs.append((fa, fb))
+    torch.cuda.synchronize()
+    ra, rb = ora_exact(oracle, wa), ora_exact(oracle, wb)
+    for fa, fb in outs:
+        assert np.abs(fa.cpu().numpy() - ra).max() <= TOL64
+        assert np.abs(fb.cpu().numpy() - rb).max() <= TOL64
