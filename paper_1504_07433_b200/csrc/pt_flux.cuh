@@ -61,7 +61,8 @@ struct FluxArgs {
   int tile_len;            // exposures per tile (multiple of 256, <= kMaxTileLen)
   int tiles_per_pv;
   int64_t n_tiles;
-  unsigned long long* sched;   // [0] next tile to hand out (beyond the first one per warp), [1] warps that have finished
+  unsigned long long* sched;   // scheduler slot: [0] global tile ticket, [1] warps that have finished, [2+pv] per-pv tickets
+  int per_pv;                  // 1: warps stay on one parameter vector and take its tiles from sched[2+pv] (n_pv small)
   // supersample accumulation (fixed point)
   int fx_bits;             // 61 - ceil(log2 n_ss): a sum of n_ss values below 2^eb fits an int64 at scale 2^(fx_bits-eb)
   double fx_scale;         // 2^fx_bits (basis values are <= 1)
@@ -107,6 +108,11 @@ struct WarpState {
   uint8_t item_ring[kItemQ];    // n_ss == 1: PvRec index
   uint16_t expq[kExpQ];
   double coefc[3 * kCoefCache];
+};
+
+// Ring positions of one warp.  They are warp-uniform and live in registers: every stage is inlined at its single call
+// site in the kernel's work loop.
+struct WarpCtr {
   int qhead, qcount;            // exposure ring
   int ihead, icount;            // item ring
   int slot_next;                // next slot to hand out (mod kSlots)
@@ -235,12 +241,25 @@ __device__ __forceinline__ double pow2i(int s) {
 // Row validation, k̂ (summed in index order, R9), orbit constants and phase window (pv_setup_orbit), combine
 // coefficients coef = g (1-c)/N, g c/N, g u2/N with g = k_j²/k̂², table indices, window-test constants.
 template <int MODE, bool NPB1, typename OutT>
-__device__ __noinline__ void tile_setup(const FluxArgs& A, WarpState& ws, int ring, int64_t tile) {
+__device__ __noinline__ void tile_setup(const FluxArgs& A, WarpState& ws, int ring, int64_t pv, int chunk, int reuse) {
   const int lane = threadIdx.x & 31;
   PvRec& r = ws.pv[ring];
-  const int64_t pv = tile / A.tiles_per_pv;
-  const int chunk = (int)(tile - pv * A.tiles_per_pv);
   const int n_pb = NPB1 ? 1 : A.n_pb;
+  if (reuse >= 0) {   // same parameter vector as the previous tile of this warp: copy its record, move the tile pointers
+    const int64_t e0 = (int64_t)chunk * A.tile_len;
+    if (reuse != ring) {
+      const double* src = reinterpret_cast<const double*>(&ws.pv[reuse]);
+      double* dst = reinterpret_cast<double*>(&r);
+      for (int i = lane; i < (int)(sizeof(PvRec) / sizeof(double)); i += 32) dst[i] = src[i];
+      __syncwarp();
+    }
+    if (lane == 0) {
+      r.tb = A.times + pv * A.t_stride_pv + e0;
+      r.ob = (char*)A.flux + ((pv * n_pb) * A.n_t + e0) * (int64_t)sizeof(OutT);
+    }
+    __syncwarp();
+    return;
+  }
   const double* row = A.params + pv * (6 + 3 * (int64_t)n_pb);
   bool ok = true;
   double ksum = 0.0, N0 = 1.0;
@@ -339,10 +358,10 @@ __device__ __forceinline__ bool in_window2(double t, double invP, double c0, dou
 #define PT_BASIS_INLINE __forceinline__
 #endif
 template <int MODE, bool NPB1, bool SS1, typename OutT>
-__device__ PT_BASIS_INLINE void basis_round(const FluxArgs& A, WarpState& ws, int n) {
+__device__ PT_BASIS_INLINE void basis_round(const FluxArgs& A, WarpState& ws, WarpCtr& C, int n) {
   const int lane = threadIdx.x & 31;
   const bool act = lane < n;
-  const int ihead = ws.ihead;
+  const int ihead = C.ihead;
   const int idx = (ihead + lane) & (kItemQ - 1);
   if (SS1) {
     if (act) {
@@ -408,17 +427,15 @@ __device__ PT_BASIS_INLINE void basis_round(const FluxArgs& A, WarpState& ws, in
     }
   }
   __syncwarp();
-  if (lane == 0) {
-    ws.ihead = (ihead + n) & (kItemQ - 1);
-    ws.icount -= n;
-  }
-  __syncwarp();
+  C.ihead = (ihead + n) & (kItemQ - 1);
+  C.icount -= n;
 }
 
 // ---------------------------------------------------------------------------------------------------- z-stage
 // Expand the first nb (<= EPW = 32/G) queued exposures of the current tile into subsamples, G = min(n_ss,32) lanes each:
 // pinned subsample time and phase fold (H1, H2), orbit, in-transit test; compacts the in-transit subsamples into
-// the item queue.  Runs basis rounds itself whenever 32 items are waiting.
+// the item queue.  One call is one z-round; for n_ss > 32 an exposure takes several calls (`ms0`, `msid` carry the
+// subsample offset and the slot across them) so that the kernel can run basis rounds in between from its single call site.
 // Per-lane constants of the z-stage, computed once per kernel: group (exposure) and subsample index of the lane, and the
 // pinned subsample offset (H2) when one round covers all subsamples.
 struct LaneCtx {
@@ -427,17 +444,17 @@ struct LaneCtx {
 };
 
 template <int MODE, bool NPB1, bool SS1, typename OutT>
-__device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, const LaneCtx& L, int nb) {
+__device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, WarpCtr& C, const LaneCtx& L, int nb, int& ms0, int& msid) {
   const int lane = threadIdx.x & 31;
   const unsigned lt = (1u << lane) - 1u;
-  const int cur = ws.cur;
+  const int cur = C.cur;
   const PvRec& r = ws.pv[cur];
   const int n_pb = NPB1 ? 1 : A.n_pb;
   const int n_ss = SS1 ? 1 : A.n_ss;
   const int G = n_ss < 32 ? n_ss : 32;
   const int grp = L.grp, g = L.g;
   const bool act = grp < nb;
-  const int qhead = ws.qhead;
+  const int qhead = C.qhead;
   const uint32_t e = act ? ws.expq[(qhead + grp) & (kExpQ - 1)] : 0u;
   const double t = act ? __ldg(r.tb + e) : 0.0;
   const double khat = r.c.khat;
@@ -456,19 +473,16 @@ __device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, const 
         store_one<NPB1, OutT>(ob + e, A.n_t, n_pb);
       }
     }
-    __syncwarp();
-    if (lane == 0) {
-      ws.qhead = (qhead + nb) & (kExpQ - 1);
-      ws.qcount -= nb;
-    }
-    __syncwarp();
+    C.qhead = (qhead + nb) & (kExpQ - 1);
+    C.qcount -= nb;
     return;
   } else {
     const bool multi = n_ss > 32;             // one exposure per round, several sub-rounds of 32 subsamples
     const unsigned gmask = (G == 32 ? 0xffffffffu : ((1u << G) - 1u)) << (grp * G);
     const unsigned below = (grp * G >= 32) ? 0xffffffffu : ((1u << (grp * G)) - 1u);   // lanes of earlier groups
-    int sid = -1;
-    for (int s0 = 0; s0 < n_ss; s0 += 32) {
+    const int s0 = multi ? ms0 : 0;
+    int sid = multi ? msid : -1;
+    {
       const int s = s0 + g;
       bool p = false;
       double zs = 0.0;
@@ -483,7 +497,7 @@ __device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, const 
         const int cnt = __popc(m & gmask);
         const bool has = act && cnt > 0;
         const unsigned hm = __ballot_sync(0xffffffffu, has && g == 0);
-        sid = (ws.slot_next + __popc(hm & below)) & (kSlots - 1);
+        sid = (C.slot_next + __popc(hm & below)) & (kSlots - 1);
         nalloc = __popc(hm);
         if (act && g == 0) {
           if (has) {
@@ -496,7 +510,7 @@ __device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, const 
         }
       } else if (m) {
         if (sid < 0) {
-          sid = ws.slot_next & (kSlots - 1);
+          sid = C.slot_next & (kSlots - 1);
           nalloc = 1;
           if (lane == 0) {
             Slot& sl = ws.slots[sid];
@@ -508,19 +522,20 @@ __device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, const 
         if (lane == 0) ws.slots[sid].remaining += __popc(m);
       }
       if (p) {
-        const int pos = (ws.ihead + ws.icount + __popc(m & lt)) & (kItemQ - 1);
+        const int pos = (C.ihead + C.icount + __popc(m & lt)) & (kItemQ - 1);
         ws.item_z[pos] = zs;
         ws.item_tag[pos] = (uint16_t)sid;
       }
       __syncwarp();
-      if (lane == 0) {
-        ws.icount += __popc(m);
-        ws.slot_next = (ws.slot_next + nalloc) & (kSlots - 1);
-      }
-      __syncwarp();
-      if (multi) while (ws.icount >= 32) basis_round<MODE, NPB1, SS1, OutT>(A, ws, 32);
+      C.icount += __popc(m);
+      C.slot_next = (C.slot_next + nalloc) & (kSlots - 1);
     }
     if (multi) {
+      ms0 = s0 + 32;
+      msid = sid;
+      if (ms0 < n_ss) return;                 // more sub-rounds of this exposure to come
+      ms0 = 0;
+      msid = -1;
       if (sid < 0) {
         if (lane == 0) store_one<NPB1, OutT>(ob + e, A.n_t, n_pb);
       } else if (lane == 0) {
@@ -535,21 +550,38 @@ __device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, const 
       }
     }
     __syncwarp();
-    if (lane == 0) {
-      ws.qhead = (qhead + nb) & (kExpQ - 1);
-      ws.qcount -= nb;
-    }
-    __syncwarp();
+    C.qhead = (qhead + nb) & (kExpQ - 1);
+    C.qcount -= nb;
   }
-  if (!SS1) while (ws.icount >= 32) basis_round<MODE, NPB1, SS1, OutT>(A, ws, 32);
 }
 
-// Drain the item queue completely (ragged last batch): before a PvRec that live items refer to is overwritten, and at
-// the end of the kernel.
-template <int MODE, bool NPB1, bool SS1, typename OutT>
-__device__ __forceinline__ void drain_items(const FluxArgs& A, WarpState& ws) {
-  if (SS1) return;   // the n_ss == 1 path never queues items
-  while (ws.icount > 0) basis_round<MODE, NPB1, SS1, OutT>(A, ws, min(ws.icount, 32));
+// Per-pv scheduling: find the next parameter vector after `pv` (cyclically) that still has tiles and take one.
+// Lanes look at 32 counters at a time (plain loads: a stale value only costs a wasted ticket), then one ticket is drawn
+// from the first candidate; a counter only ever grows, so an exhausted parameter vector stays exhausted.
+__device__ __forceinline__ bool next_pv(const FluxArgs& A, int64_t& pv, int& chunk) {
+  const int lane = threadIdx.x & 31;
+  const int64_t n_pv = A.n_pv;
+  const unsigned long long tpp = (unsigned long long)A.tiles_per_pv;
+  for (int64_t off = 1; off < n_pv; off += 32) {
+    const int64_t cand = (pv + off + lane) % n_pv;
+    const bool in_range = off + lane < n_pv;
+    const unsigned long long seen = in_range ? *((volatile unsigned long long*)(A.sched + 2 + cand)) : tpp;
+    unsigned avail = __ballot_sync(0xffffffffu, seen < tpp);
+    while (avail) {
+      const int src = __ffs(avail) - 1;
+      avail &= avail - 1u;
+      const int64_t target = (pv + off + src) % n_pv;
+      unsigned long long got = 0;
+      if (lane == 0) got = atomicAdd(A.sched + 2 + target, 1ULL);
+      got = __shfl_sync(0xffffffffu, got, 0);
+      if (got < tpp) {
+        pv = target;
+        chunk = (int)got;
+        return true;
+      }
+    }
+  }
+  return false;
 }
 
 // ---------------------------------------------------------------------------------------------------- the kernel
@@ -561,10 +593,8 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
   __shared__ WarpState s_ws[kWarpsPerBlock];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   WarpState& ws = s_ws[warp];
-  if (lane == 0) {
-    ws.qhead = 0; ws.qcount = 0; ws.ihead = 0; ws.icount = 0; ws.slot_next = 0; ws.cur = 0;
-  }
-  __syncwarp();
+  WarpCtr C;
+  C.qhead = 0; C.qcount = 0; C.ihead = 0; C.icount = 0; C.slot_next = 0; C.cur = 0;
   const int n_pb = NPB1 ? 1 : A.n_pb;
   const int n_ss = SS1 ? 1 : A.n_ss;
   const int EPW = 32 / (n_ss < 32 ? n_ss : 32);
@@ -578,42 +608,82 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
   }
   const int64_t gw = (int64_t)blockIdx.x * kWarpsPerBlock + warp, nw = (int64_t)gridDim.x * kWarpsPerBlock;
 
-  // Tiles are dealt dynamically: a warp starts with tile `gw` and fetches every further one from a global counter (the
-  // fetch is issued before the current tile is processed, so its latency is hidden).  The last warp to finish resets the
-  // counter pair for the next launch that uses this scheduler slot.
-  int64_t tile = gw;
-  while (tile < A.n_tiles) {
-    unsigned long long fetched = 0;
-    if (lane == 0) fetched = atomicAdd(A.sched, 1ULL);
-    // the PvRec this tile will use must not be referenced by queued subsamples any more
-    const int ring = NPB1 ? ((ws.cur + 1) & (kPvRing - 1)) : 0;
-    if (!SS1 && ws.icount > 0) {
-      bool clash = true;
-      if (NPB1) {
-        const int ih = ws.ihead;
-        const int oldest = SS1 ? (int)ws.item_ring[ih] : (int)ws.slots[ws.item_tag[ih]].ring;
-        clash = (oldest == ring);
+  // Tiles are dealt dynamically from counters in the launch's scheduler slot; the next ticket is always drawn before the
+  // current tile is processed, so the atomic's latency is hidden.
+  //   global mode: one counter over all (pv, chunk) tiles; a warp starts with tile `gw`.
+  //   per-pv mode (few parameter vectors, several tiles each): one counter per parameter vector; a warp stays on its
+  //     parameter vector (setup done once, later tiles only move the tile pointers) and moves on to the next one that has
+  //     tiles left when it is exhausted, so fast parameter vectors lend their warps to slow ones.
+  // The last warp to finish zeroes the slot for the next launch that uses it.
+  const int tpp = A.tiles_per_pv;
+  int64_t pv_cur = 0, last_pv = -1;
+  int chunk_cur = 0, last_ring = -1;
+  bool have;
+  if (!A.per_pv) {
+    have = gw < A.n_tiles;
+    pv_cur = gw / tpp;
+    chunk_cur = (int)(gw - pv_cur * tpp);
+  } else {
+    pv_cur = gw % A.n_pv;
+    unsigned long long f0 = 0;
+    if (lane == 0) f0 = atomicAdd(A.sched + 2 + pv_cur, 1ULL);
+    f0 = __shfl_sync(0xffffffffu, f0, 0);
+    have = f0 < (unsigned long long)tpp;
+    chunk_cur = (int)f0;
+    if (!have) have = next_pv(A, pv_cur, chunk_cur);
+  }
+
+  // The warp's work loop is a small state machine so that every stage has exactly ONE call site (one copy of its code:
+  // the stages are large, and two inlined copies of the basis functions need not round identically).  Priority: a full
+  // basis round, then a z-round, then the next piece of streaming / the next tile.
+  enum { PH_NEWTILE, PH_STREAM, PH_EXIT };
+  int phase = have ? PH_NEWTILE : PH_EXIT;
+  bool drain_all = false;        // empty the item queue (ragged last round) before going on
+  int keep = EPW;                // z-rounds run while the exposure ring holds at least this many entries
+  int ms0 = 0, msid = -1;        // n_ss > 32: sub-round state of the exposure being expanded
+  uint32_t base = 0, n_e = 0;
+  unsigned long long fetched = 0;
+  const double* __restrict__ tb = nullptr;
+  OutT* __restrict__ ob = nullptr;
+  double w_invP = 0.0, w_c0 = 0.0, w_half = 0.0;
+
+  for (;;) {
+    if (!SS1) {
+      const int ic = C.icount;
+      if (ic >= 32 || (drain_all && ic > 0)) {
+        basis_round<MODE, NPB1, SS1, OutT>(A, ws, C, min(ic, 32));
+        continue;
       }
-      if (clash) drain_items<MODE, NPB1, SS1, OutT>(A, ws);
+      drain_all = false;
     }
-    tile_setup<MODE, NPB1, OutT>(A, ws, ring, tile);
-    if (lane == 0) ws.cur = ring;
-    __syncwarp();
-    const PvRec& r = ws.pv[ring];
-    const int chunk = (int)(tile % A.tiles_per_pv);
-    const uint32_t n_e = (uint32_t)min((int64_t)A.tile_len, A.n_t - (int64_t)chunk * A.tile_len);
-    const double* __restrict__ tb = r.tb;
-    OutT* __restrict__ ob = (OutT*)r.ob;
-
-    if (r.c.flags & PV_BAD) {
-      for (int j = 0; j < n_pb; ++j)
-        for (uint32_t e = lane; e < n_e; e += 32) ob[(int64_t)j * A.n_t + e] = (OutT)nan64();
-      tile = nw + (int64_t)__shfl_sync(0xffffffffu, fetched, 0);
-      continue;
+    {
+      const int qc = C.qcount;
+      if (qc >= keep) {
+        expand<MODE, NPB1, SS1, OutT>(A, ws, C, L, min(qc, EPW), ms0, msid);
+        continue;
+      }
     }
-    const double w_invP = r.c.invP, w_c0 = r.w_c0, w_half = r.w_half;
-
-    for (uint32_t base = 0; base < n_e; base += kSuper) {
+    if (phase == PH_STREAM) {
+      if (base >= n_e) {
+        // tile finished (the exposure ring is empty: keep was 1).  Multi-passband: the coefficient cache belongs to this
+        // parameter vector, so the item queue is emptied too.
+        if (!NPB1 && !SS1 && C.icount > 0) { drain_all = true; continue; }
+        const unsigned long long nf = __shfl_sync(0xffffffffu, fetched, 0);
+        if (!A.per_pv) {
+          const int64_t tile = nw + (int64_t)nf;
+          have = tile < A.n_tiles;
+          pv_cur = tile / tpp;
+          chunk_cur = (int)(tile - pv_cur * tpp);
+        } else if (nf < (unsigned long long)tpp) {
+          chunk_cur = (int)nf;
+        } else {
+          have = next_pv(A, pv_cur, chunk_cur);
+        }
+        phase = have ? PH_NEWTILE : PH_EXIT;
+        continue;
+      }
+      // ---- stream super-groups of kUnroll x 32 lanes x V exposures until a z-round is due or the tile ends
+      do {
       unsigned inw = 0;                                          // bit (u*V+v): exposure (u,v) of this lane is in the window
       if (base + kSuper <= n_e) {                                // warp-uniform
         double t[kUnroll][V];
@@ -661,7 +731,7 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
           if (lane >= o) incl += up;
         }
         const int total = __shfl_sync(0xffffffffu, incl, 31);
-        int pos = ws.qhead + ws.qcount + incl - cnt;
+        int pos = C.qhead + C.qcount + incl - cnt;
         while (inw) {
           const int b = __ffs(inw) - 1;
           inw &= inw - 1u;
@@ -669,22 +739,52 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
           ++pos;
         }
         __syncwarp();
-        if (lane == 0) ws.qcount += total;
-        __syncwarp();
+        C.qcount += total;
       }
-      // full z-rounds; at the end of the tile the exposure ring is emptied (it holds this tile's indices), ragged
-      const int keep = (base + kSuper >= n_e) ? 1 : EPW;
-      while (ws.qcount >= keep) expand<MODE, NPB1, SS1, OutT>(A, ws, L, min(ws.qcount, EPW));
+      base += kSuper;
+      } while (base < n_e && C.qcount < EPW);
+      if (base >= n_e) keep = 1;      // end of the tile: the exposure ring holds this tile's indices, so it is emptied
+      continue;
     }
-    if (!NPB1) drain_items<MODE, NPB1, SS1, OutT>(A, ws);   // the coefficient cache belongs to this parameter vector
-    tile = nw + (int64_t)__shfl_sync(0xffffffffu, fetched, 0);
+    if (phase == PH_NEWTILE) {
+      // the PvRec this tile will use must not be referenced by queued subsamples any more
+      const int ring = NPB1 ? ((C.cur + 1) & (kPvRing - 1)) : 0;
+      if (!SS1 && C.icount > 0) {
+        bool clash = true;
+        if (NPB1) clash = ((int)ws.slots[ws.item_tag[C.ihead]].ring == ring);
+        if (clash) { drain_all = true; continue; }
+      }
+      fetched = 0;
+      if (lane == 0) fetched = atomicAdd(A.per_pv ? A.sched + 2 + pv_cur : A.sched, 1ULL);
+      tile_setup<MODE, NPB1, OutT>(A, ws, ring, pv_cur, chunk_cur, (pv_cur == last_pv) ? last_ring : -1);
+      last_pv = pv_cur;
+      last_ring = ring;
+      C.cur = ring;
+      const PvRec& r = ws.pv[ring];
+      n_e = (uint32_t)min((int64_t)A.tile_len, A.n_t - (int64_t)chunk_cur * A.tile_len);
+      tb = r.tb;
+      ob = (OutT*)r.ob;
+      base = 0;
+      keep = EPW;
+      if (r.c.flags & PV_BAD) {
+        for (int j = 0; j < n_pb; ++j)
+          for (uint32_t e = lane; e < n_e; e += 32) ob[(int64_t)j * A.n_t + e] = (OutT)nan64();
+        base = n_e;       // nothing to stream
+        keep = 1;
+      }
+      w_invP = r.c.invP; w_c0 = r.w_c0; w_half = r.w_half;
+      phase = PH_STREAM;
+      continue;
+    }
+    // PH_EXIT
+    if (!SS1 && C.icount > 0) { drain_all = true; continue; }
+    break;
   }
-  drain_items<MODE, NPB1, SS1, OutT>(A, ws);
   if (lane == 0) {
     const unsigned long long done = atomicAdd(A.sched + 1, 1ULL);
-    if (done == (unsigned long long)nw - 1ULL) {   // every warp has taken its last ticket: nobody reads the pair any more
-      A.sched[0] = 0ULL;
-      A.sched[1] = 0ULL;
+    if (done == (unsigned long long)nw - 1ULL) {   // every warp has taken its last ticket: nobody reads the slot any more
+      const int64_t nwords = 2 + (A.per_pv ? A.n_pv : 0);
+      for (int64_t i = 0; i < nwords; ++i) A.sched[i] = 0ULL;
     }
   }
 }

@@ -14,11 +14,12 @@ namespace pt {
 
 static std::atomic<int64_t> g_launches{0};
 
-// Scheduler slots of the flux kernel (tile counter + finished-warp counter each).  A launch takes the next slot in a ring;
+// Scheduler slots of the flux kernel (tile counters + finished-warp counter each).  A launch takes the next slot in a ring;
 // the kernel leaves its slot zeroed when it ends, so a slot is clean again long before the ring comes back to it (that
 // would need kSchedSlots launches in flight at once).  This is the only state the library keeps on the device.
-constexpr int kSchedSlots = 4096;
-__device__ unsigned long long g_sched[kSchedSlots][2];
+constexpr int kSchedSlots = 1024;
+constexpr int kSchedWords = 1024;   // [0] global ticket, [1] finished warps, [2 + pv] per-parameter-vector tickets
+__device__ unsigned long long g_sched[kSchedSlots][kSchedWords];
 static std::atomic<uint64_t> g_sched_seq{0};
 
 static unsigned long long* sched_slot() {
@@ -32,7 +33,7 @@ static unsigned long long* sched_slot() {
     b = (unsigned long long*)p;
     base[dev].store(b);
   }
-  return b + 2 * (g_sched_seq.fetch_add(1) % kSchedSlots);
+  return b + (size_t)kSchedWords * (g_sched_seq.fetch_add(1) % kSchedSlots);
 }
 
 // S1-S2 alone: signed projected separation of every subsample.
@@ -154,6 +155,7 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   const int64_t tpp = (n_t + tl - 1) / tl;
   if (tpp > 0x7fffffff || (double)tpp * (double)n_pv > 9.0e18) return PT_ERR_SIZE;
   A.tile_len = (int)tl; A.tiles_per_pv = (int)tpp; A.n_tiles = n_pv * tpp;
+  A.per_pv = (n_pv <= kSchedWords - 2 && tpp >= 2) ? 1 : 0;
   int lg = 0;
   while (((int64_t)1 << lg) < (int64_t)n_ss) ++lg;
   A.fx_bits = 61 - lg;
