@@ -119,18 +119,28 @@ __device__ __forceinline__ double orbit_z_signed(const PvConst& c, double ph) {
   return B > 0.0 ? z : -z;
 }
 
-// Mean anomaly of true anomaly f (any real), reduced to (-π, π].
-__device__ inline double mean_anomaly_of_true(double f, double e) {
+// Mean anomaly of true anomaly f (|f| up to a few turns), reduced to (-π, π]: tan(E/2) = sqrt((1-e)/(1+e)) tan(f/2),
+// M = E - e sin E.  rm = sqrt(1-e), rp = sqrt(1+e).  Lean primitives (pt_math.cuh): this runs once per tile.
+__device__ __forceinline__ double mean_anomaly_of_true(double f, double e, double rm, double rp) {
   double sh, ch;
-  sincos(0.5 * f, &sh, &ch);
-  const double E = 2.0 * atan2(sqrt(1.0 - e) * sh, sqrt(1.0 + e) * ch);
-  return E - e * sin(E);
+  sincos_bounded(0.5 * f, &sh, &ch);
+  const double y = rm * sh, x = rp * ch;
+  const double E = 2.0 * copysign(atan2_pos(fabs(y), x), y);
+  double sE, cE;
+  sincos_bounded(E, &sE, &cE);
+  return fma(-e, sE, E);
+}
+
+// asin(x) for 0 <= x < 1.
+__device__ __forceinline__ double asin_unit(double x) {
+  return atan2_pos(x, sqrt_fast(fmax((1.0 - x) * (1.0 + x), 0x1p-1000)));
 }
 
 // Validate a parameter row and fill the orbit part of PvConst (khat is set by the caller beforehand).
 // `row` = [t0, P, a/R*, i, e, w, ...]; half_exp_phase = half the exposure in cycles (0 when n_ss == 1).
 __device__ __forceinline__ void pv_setup_orbit(PvConst& c, const double* row, bool row_ok, int n_ss, double t_exp) {
-  const double t0 = row[0], P = row[1], a = row[2], inc = row[3], e = row[4], w = row[5];
+  const double t0 = row[0], P = row[1], a = row[2], inc = row[3], e = row[4];
+  double w = row[5];
   int flags = 0;
   if (!row_ok || !(isfinite(t0) && isfinite(P) && isfinite(a) && isfinite(inc) && isfinite(e) && isfinite(w)) ||
       !(P > 0.0) || !(a > 0.0) || !(e >= 0.0 && e < 1.0)) {
@@ -160,10 +170,16 @@ __device__ __forceinline__ void pv_setup_orbit(PvConst& c, const double* row, bo
     hi = hi * (1.0 + 1.0e-9) + margin;
     lo = -hi;
   } else {
-    sincos(w, &c.sinw, &c.cosw);
-    c.rt1me2 = sqrt((1.0 - e) * (1.0 + e));
+    if (fabs(w) <= 1.0e3) {
+      sincos_bounded(w, &c.sinw, &c.cosw);
+    } else {
+      sincos(w, &c.sinw, &c.cosw);
+      w = atan2(c.sinw, c.cosw);              // same angle, small enough for the lean kernels below
+    }
+    const double rm = sqrt_fast(1.0 - e), rp = sqrt_fast(1.0 + e);
+    c.rt1me2 = rm * rp;
     const double ftr = 0.5 * kPi - w;
-    c.Mtr = mean_anomaly_of_true(ftr, e);
+    c.Mtr = mean_anomaly_of_true(ftr, e, rm, rp);
     // overlap needs r |cos(w+f)| < 1+k and sin(w+f) > 0.  First bound with r >= a(1-e), then tighten with the smallest
     // r on the resulting true-anomaly range (any in-transit f lies in the first range, so the second is still safe).
     const double one_k = 1.0 + k;
@@ -171,15 +187,18 @@ __device__ __forceinline__ void pv_setup_orbit(PvConst& c, const double* row, bo
     if (!(C < 1.0)) {
       flags |= PV_ALWAYS; lo = -1.0; hi = 1.0;
     } else {
-      double D = asin(C);
+      double D = asin_unit(C);
       // max of cos f over [ftr-D, ftr+D]
       const double fc = ftr - kTwoPi * rint(ftr * (1.0 / kTwoPi));   // reduce to [-π, π]
-      const double cmax = (fabs(fc) <= D) ? 1.0 : fmax(cos(fc - D), cos(fc + D));
+      double s1, c1, s2, c2;
+      sincos_bounded(fc - D, &s1, &c1);
+      sincos_bounded(fc + D, &s2, &c2);
+      const double cmax = (fabs(fc) <= D) ? 1.0 : fmax(c1, c2);
       const double rmin = a * (1.0 - e) * (1.0 + e) / fma(e, cmax, 1.0);
       C = fmin(C, one_k / rmin);
-      D = asin(C) * (1.0 + 1.0e-9) + 1.0e-9;
-      double dhi = mean_anomaly_of_true(ftr + D, e) - c.Mtr;
-      double dlo = c.Mtr - mean_anomaly_of_true(ftr - D, e);
+      D = asin_unit(C) * (1.0 + 1.0e-9) + 1.0e-9;
+      double dhi = mean_anomaly_of_true(ftr + D, e, rm, rp) - c.Mtr;
+      double dlo = c.Mtr - mean_anomaly_of_true(ftr - D, e, rm, rp);
       dhi -= kTwoPi * floor(dhi * (1.0 / kTwoPi));   // both differences are in [0, 2π)
       dlo -= kTwoPi * floor(dlo * (1.0 / kTwoPi));
       hi = dhi * (1.0 / kTwoPi) * (1.0 + 1.0e-9) + margin;
