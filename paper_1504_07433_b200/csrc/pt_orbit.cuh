@@ -20,7 +20,7 @@ enum PvFlags : int { PV_BAD = 1, PV_CIRCULAR = 2, PV_NEVER = 4, PV_ALWAYS = 8, P
 // Constants of one parameter vector (shared memory, one per block).
 struct PvConst {
   double t0, P, invP;
-  double a, cosi, e, sinw, cosw, rt1me2, Mtr;
+  double a, cosi, e, sinw, cosw, rt1me2, Mtr, sin_e, cos_e;
   double khat;
   double ph_lo, ph_hi;   // conservative phase window of the transit (cycles, relative to conjunction), sample-level
   double ex_lo, ex_hi;   // the same widened by half an exposure: exposure-level test on the exposure centre
@@ -67,27 +67,40 @@ __device__ __forceinline__ bool in_window(double t, double t0, double invP, doub
 // Eccentric anomaly from mean anomaly M in (-π, π] by Newton's method.  Starter: for e <= 0.8 the third-order
 // guess M + e sin M / (1 - sin(M+e) + sin M) (<= 6 steps); above that E0 = M ± e, which lies on the convex side of the
 // root so Newton descends monotonically (<= 12 steps at e = 0.999).
-__device__ __forceinline__ void kepler_newton(double M, double e, double* sinE, double* cosE) {
+__device__ __forceinline__ void kepler_newton(double M, double e, double sin_e, double cos_e, double* sinE, double* cosE) {
   double E;
   double sE, cE, dE;
   if (e <= 0.8) {
-    double sM, cM, sMe, cMe;
+    double sM, cM;
     sincos_bounded(M, &sM, &cM);
-    sincos_bounded(M + e, &sMe, &cMe);
+    const double sMe = fma(sM, cos_e, cM * sin_e);   // sin(M + e), (sin e, cos e) are per-orbit constants
     E = fma(e * sM, rcp_fast(1.0 - sMe + sM), M);
   } else {
     E = M + copysign(e, M);
   }
   const double tol = 0x1p-30 * (1.0 - e);
   bool conv = false;
+  sincos_bounded(E, &sE, &cE);
 #pragma unroll 1
   for (int it = 0; it < 32; ++it) {
-    sincos_bounded(E, &sE, &cE);
     const double f = E - fma(e, sE, M);
     const double fp = fma(-e, cE, 1.0);
     dE = f * rcp_fast(fp);
     E -= dE;
-    if (fabs(dE) < tol) { conv = true; break; }   // the step just applied squares the error: converged to rounding
+    const double ad = fabs(dE);
+    if (ad < tol) { conv = true; break; }   // the step just applied squares the error: converged to rounding
+    if (ad < 0x1p-7) {
+      // small step: rotate (sin E, cos E) by -dE with short series (sin through dE^5, cos through dE^6: the neglected
+      // terms are below 4e-19) instead of a full sincos
+      const double d2 = dE * dE;
+      const double sd = dE * fma(d2, fma(d2, 1.0 / 120.0, -1.0 / 6.0), 1.0);
+      const double cd = fma(d2, fma(d2, fma(d2, -1.0 / 720.0, 1.0 / 24.0), -0.5), 1.0);
+      const double ns = fma(sE, cd, -cE * sd);
+      cE = fma(cE, cd, sE * sd);
+      sE = ns;
+    } else {
+      sincos_bounded(E, &sE, &cE);
+    }
   }
   if (conv) {   // sin/cos of E - dE to first order in dE (|dE| < 1e-9: the neglected term is < 5e-19)
     *sinE = fma(-cE, dE, sE);
@@ -110,7 +123,7 @@ __device__ __forceinline__ double orbit_z_signed(const PvConst& c, double ph) {
   if (M > kC[C_PI]) M -= kC[C_TWOPI];
   if (M <= -kC[C_PI]) M += kC[C_TWOPI];
   double sE, cE;
-  kepler_newton(M, c.e, &sE, &cE);
+  kepler_newton(M, c.e, c.sin_e, c.cos_e, &sE, &cE);
   const double x = cE - c.e, y = c.rt1me2 * sE;
   const double A = c.cosw * x - c.sinw * y;   // (r/a) cos(w+f)
   const double B = c.sinw * x + c.cosw * y;   // (r/a) sin(w+f)
@@ -158,7 +171,7 @@ __device__ __forceinline__ void pv_setup_orbit(PvConst& c, const double* row, bo
   double lo, hi;
   if (e == 0.0) {
     flags |= PV_CIRCULAR;
-    c.sinw = 0.0; c.cosw = 1.0; c.rt1me2 = 1.0; c.Mtr = 0.0;
+    c.sinw = 0.0; c.cosw = 1.0; c.rt1me2 = 1.0; c.Mtr = 0.0; c.sin_e = 0.0; c.cos_e = 1.0;
     // overlap needs a²(cos²i + sin²i sin²φ) < (1+k)² and cos φ > 0
     const double ci2 = c.cosi * c.cosi;
     const double si2 = 1.0 - ci2;
@@ -176,6 +189,7 @@ __device__ __forceinline__ void pv_setup_orbit(PvConst& c, const double* row, bo
       sincos(w, &c.sinw, &c.cosw);
       w = atan2(c.sinw, c.cosw);              // same angle, small enough for the lean kernels below
     }
+    sincos_bounded(e, &c.sin_e, &c.cos_e);
     const double rm = sqrt_fast(1.0 - e), rp = sqrt_fast(1.0 + e);
     c.rt1me2 = rm * rp;
     const double ftr = 0.5 * kPi - w;
