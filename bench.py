@@ -35,6 +35,11 @@ ALG_PER_COMBINE = 5.0         # per (exposure, passband): 3 FMA + mul + sub
 ALG_PER_TRANSIT_CIRC = 650.0  # in-transit subsample, circular orbit: z + case split + λe, λd, ηd
 ALG_PER_TRANSIT_ECC = 900.0   # the same with the Newton–Kepler solve
 FP64_LANES_PER_SM, N_SM = 64, 148
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/r1c_ncu_*.md);
+# a kernel's output that is still in L2 when the capture ends is not in its figure (configs[1]: 30.7 MB of flux < 126 MB L2).
+TRAFFIC_EXACT_CONFIG2 = 557.824e3 + 11.008e3
+TRAFFIC_INTERP_F32 = 514.131456e6 + 3.232009e9
+TRAFFIC_DENSE = 134.581504e6 + 88.507392e6
 
 
 def _peaks():
@@ -248,7 +253,7 @@ def run_ours(args):
         extra["dense"] = {"workload": "configs[4]-like population, 4096 pv x 4096 per-pv times, all within 0.75 T14, e~U(0,0.6)",
                           "value": wd.n_eval / t_d, "unit": UNIT, "ms": t_d * 1e3, "in_transit_frac": n_in_d / wd.n_eval,
                           "fp64_frac_of_model_peak": alg_d / t_d / fp64_model_peak,
-                          "fp64_frac_of_measured_peak": alg_d / t_d / fp64_meas_peak}
+                          "fp64_frac_of_measured_peak": alg_d / t_d / fp64_meas_peak, "traffic": TRAFFIC_DENSE}
         # fp32-output variant on the same workload
         do32 = torch.empty((wd.n_pv, 1, wd.n_t), dtype=torch.float32, device=dev)
         t_d32 = _time_steps(lambda: pt.pt_ma_quad_exact(dt_, dp_, dtype=torch.float32, out=do32), 10, 3, flush, 1) / 10
@@ -269,7 +274,8 @@ def run_ours(args):
             bytes_alg = wi.n_pv * wi.n_t * 8.0      # the flux write; shared times (0.8 MB) and the table live in L2
             res_i[name] = {"value": wi.n_eval / t_i, "unit": UNIT, "ms": t_i * 1e3, "table_build_ms": t_build * 1e3,
                            "roofline": {"bound": "hbm", "achieved": bytes_alg / t_i / 1e9, "peak": peaks["hbm_gbs"],
-                                        "unit": "GB/s", "frac": bytes_alg / t_i / 1e9 / peaks["hbm_gbs"], "traffic": None,
+                                        "unit": "GB/s", "frac": bytes_alg / t_i / 1e9 / peaks["hbm_gbs"],
+                                        "traffic": TRAFFIC_INTERP_F32 if name == "f32_table" else None,
                                         "peak_source": peaks["source"]}}
             del tb
         res_i["workload"] = "BASELINE.json configs[3]: 4096 pv x 100000 times, table 401 x 12501, fp64 flux (3.28 GB/launch > L2)"
@@ -296,8 +302,9 @@ def run_ours(args):
                        "l2": "256 MiB buffer rewritten between timed steps (L2 flushed); per-step CUDA events"},
             "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e,
             "roofline": {"bound": "alu", "achieved": ach * 2 / 1e12, "peak": fp64_model_peak * 2 / 1e12,
-                         "unit": "TFLOP/s", "frac": ach / fp64_model_peak, "traffic": None,
-                         "kernel": "flux_kernel<0,double>", "in_transit_evals": n_in, "alg_fp64_inst_per_launch": alg_inst,
+                         "unit": "TFLOP/s", "frac": ach / fp64_model_peak, "traffic": TRAFFIC_EXACT_CONFIG2,
+                         "traffic_source": "profiles/r1c_ncu_exact_config2.md (bytes per launch)",
+                         "kernel": "flux_kernel<0,2,1,0,double>", "in_transit_evals": n_in, "alg_fp64_inst_per_launch": alg_inst,
                          "peak_source": "model: 148 SM x 64 FP64 lanes x sm_max_mhz x 2 flop (DESIGN.md §6)",
                          "fp64_peak_measured_tflops": fp64_meas_peak * 2 / 1e12,
                          "frac_of_measured_dfma_peak": ach / fp64_meas_peak,

@@ -12,7 +12,9 @@
  *   - Pointers named d_* are DEVICE pointers (e.g. torch tensor .data_ptr()); pointers named h_* are HOST pointers.
  *     The caller owns all of them.  The d_* entry points never allocate, free, copy to the host or synchronise: they
  *     validate their arguments, enqueue kernels on `stream` (a cudaStream_t passed as void*; NULL = default stream)
- *     and return.  They hold no global state and are re-entrant.
+ *     and return.  They are re-entrant (any thread, any stream).  The only state the library keeps is a ring of
+ *     scheduler slots in device memory (tile counters of the persistent flux kernel); every launch takes the next slot
+ *     and leaves it zeroed, so launches on different streams never share one.
  *   - Parameter rows (`d_params`, row-major [n_pv][6 + 3 n_pb] doubles):
  *         [ t0, P, a/R*, i, e, w,  k_0, u1_0, u2_0,  k_1, u1_1, u2_1, ... ]
  *     t0 = time of inferior conjunction, P = period (same unit as the times), a/R* = scaled semi-major axis,
@@ -45,7 +47,7 @@ extern "C" {
 #endif
 
 enum { PT_OK = 0, PT_ERR_NULL = 1, PT_ERR_SIZE = 2, PT_ERR_DTYPE = 3, PT_ERR_TABLE = 4, PT_ERR_CUDA = 5 };
-enum { PT_F64 = 0, PT_F32 = 1 };                          /* arithmetic + storage type of the flux / of a table */
+enum { PT_F64 = 0, PT_F32 = 1 };                          /* storage type of the flux / of a table (arithmetic is fp64) */
 enum { PT_ST_BAD_PARAM = 1, PT_ST_K_OUT_OF_TABLE = 2 };   /* bits OR-ed into d_status[0] */
 
 /* Interpolation table descriptor (host struct holding a device pointer).  Layout [n_k][n_z][n_fn], n_fn = 3
@@ -67,8 +69,10 @@ int pt_orbit_z(const double* d_times, int64_t n_t, int64_t t_stride_pv, const do
                int32_t n_pb, int32_t n_ss, double t_exp, double* d_z, void* stream);
 
 /* S0-S7: exact quadratic Mandel–Agol flux (Eq. 13 with P:L143).
- *   dtype  PT_F64: all arithmetic fp64, d_flux is double.  PT_F32: time -> phase -> z in fp64, the case split, basis
- *          functions and combine in fp32 (fp64 only where fp32 cannot hold 2e-6, H5), d_flux is float.
+ *   dtype  PT_F64: d_flux is double.  PT_F32: d_flux is float (the fp32 variant of BASELINE.json, gate 2e-6 abs): the
+ *          arithmetic stays fp64 up to the store, because the closed forms lose 2-3 digits to cancellation near the
+ *          contacts and for small k, which fp32 cannot afford at 2e-6 (R18); what fp32 buys is half the
+ *          output traffic, which is what bounds the out-of-transit and interpolated paths.
  *   d_flux [n_pv][n_pb][n_t], time fastest.   d_status: NULL or 2 x int32 (see above). */
 int pt_ma_quad_exact(const double* d_times, int64_t n_t, int64_t t_stride_pv, const double* d_params, int64_t n_pv,
                      int32_t n_pb, int32_t n_ss, double t_exp, int32_t dtype, void* d_flux, int32_t* d_status,
@@ -85,7 +89,7 @@ int pt_ma_table_build(double k_min, double k_max, int32_t n_k, double z_max, int
 /* S9 (+S0-S3, S6, S7): interpolated quadratic Mandel–Agol flux ("bilinear interpolation"):
  *   rk = (k̂-k_min)/dk, ik = min(floor(rk), n_k-2), fk = rk-ik; rz = z/dz, iz = min(floor(rz), n_z-2), fz = rz-iz;
  *   v = (1-fk)[(1-fz)T[ik][iz] + fz T[ik][iz+1]] + fk[(1-fz)T[ik+1][iz] + fz T[ik+1][iz+1]] for each function, then
- *   Eq. 13.  Samples with z >= 1+k̂ never touch the table.  `dtype` is the arithmetic/output type as above; the table's
+ *   Eq. 13.  Samples with z >= 1+k̂ never touch the table.  `dtype` is the output type as above; the table's
  *   own storage type is in the descriptor.  A parameter vector whose k̂ lies outside [k_min, k_min+(n_k-1)dk] is
  *   evaluated by the exact device path and PT_ST_K_OUT_OF_TABLE is raised (paper silent; R13).
  *   PT_ERR_TABLE: descriptor inconsistent (NULL data, n_k/n_z < 2, n_fn not 3/4, dk/dz <= 0, unknown dtype). */
