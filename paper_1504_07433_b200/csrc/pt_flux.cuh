@@ -721,17 +721,19 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
           }
         }
       }
-      // append the in-window exposures to the exposure ring: warp prefix sum of the per-lane counts
+      // append the in-window exposures to the exposure ring.  A lane rarely holds more than two of them (its exposures
+      // are 32*V apart), so the exclusive prefix of the per-lane counts is built from one ballot per count level.
       if (__reduce_or_sync(0xffffffffu, inw)) {
+        const unsigned lt = (1u << lane) - 1u;
         const int cnt = __popc(inw);
-        int incl = cnt;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-          const int up = __shfl_up_sync(0xffffffffu, incl, o);
-          if (lane >= o) incl += up;
+        int excl = 0, total = 0;
+        for (int level = 1;; ++level) {
+          const unsigned m = __ballot_sync(0xffffffffu, cnt >= level);
+          if (m == 0) break;
+          excl += __popc(m & lt);
+          total += __popc(m);
         }
-        const int total = __shfl_sync(0xffffffffu, incl, 31);
-        int pos = C.qhead + C.qcount + incl - cnt;
+        int pos = C.qhead + C.qcount + excl;
         while (inw) {
           const int b = __ffs(inw) - 1;
           inw &= inw - 1u;
