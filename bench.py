@@ -281,6 +281,25 @@ def run_ours(args):
         res_i["workload"] = "BASELINE.json configs[3]: 4096 pv x 100000 times, table 401 x 12501, fp64 flux (3.28 GB/launch > L2)"
         extra["interp"] = res_i
         del it_, ip_, io
+    if rank == 0 and "chi2" in sections:
+        # -------------------------------------------------------------- fused likelihood (S§8(f) NEXT-1): no flux is written
+        res_c = {}
+        rng = np.random.default_rng(1504)
+        for name, wl, use_table in (("config2", inputs.config2(), False), ("config4_exact", inputs.config4(), False),
+                                    ("config4_interp", inputs.config4(), True)):
+            ct, cp = to_dev(wl.times), to_dev(wl.params)
+            truth = pt.pt_ma_quad_exact(ct, cp[:1].contiguous(), 1, wl.n_ss, wl.t_exp)[0]
+            obs = (truth + 2e-4 * torch.from_numpy(rng.standard_normal((1, wl.n_t))).to(dev)).contiguous()
+            isig = torch.full_like(obs, 1.0 / 2e-4)
+            tbl = pt.pt_ma_table_build(dtype=torch.float32, n_fn=4, **wl.table) if use_table else None
+            co = torch.empty(wl.n_pv, dtype=torch.float64, device=dev)
+            t_c = _time_steps(lambda: pt.pt_ma_quad_chi2(ct, cp, obs, isig, 1, wl.n_ss, wl.t_exp, table=tbl, out=co),
+                              10, 3, flush, 1) / 10
+            res_c[name] = {"value": wl.n_eval / t_c, "unit": UNIT, "ms": t_c * 1e3, "launches_per_call": 2}
+            del ct, cp, obs, isig, co, tbl
+        res_c["note"] = ("pt_ma_quad_chi2: chi2[pv] against one data set; out-of-window exposures cost a window test and no "
+                         "memory traffic (times are L2-resident), so the flux-store roofline does not apply")
+        extra["chi2"] = res_c
     if rank == 0 and "cpu" in sections:
         # -------------------------------------------------------------- CPU baseline: the oracle as it stands
         from oracle import pt_oracle
@@ -352,8 +371,8 @@ def main():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--sections", default="scaled,dense,interp,cpu",
-                    help="extra sections to run besides the headline: any of scaled,dense,interp,cpu (or 'none')")
+    ap.add_argument("--sections", default="scaled,dense,interp,chi2,cpu",
+                    help="extra sections to run besides the headline: any of scaled,dense,interp,chi2,cpu (or 'none')")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

@@ -97,6 +97,19 @@ int pt_ma_quad_interp(const pt_table* table, const double* d_times, int64_t n_t,
                       const double* d_params, int64_t n_pv, int32_t n_pb, int32_t n_ss, double t_exp, int32_t dtype,
                       void* d_flux, int32_t* d_status, void* stream);
 
+/* Fused likelihood (the paper's "offload z and likelihood to the GPU" variant):
+ *   chi2[pv] = sum over passbands j and exposures t of ((obs[j][t] - F_pv[j][t]) * isig[j][t])²
+ * with F the flux of pt_ma_quad_exact (table == NULL) or pt_ma_quad_interp (table != NULL); no flux is written.
+ *   d_obs, d_isig  [n_pb][n_t] doubles: observed flux and 1/sigma, ONE data set shared by all parameter vectors (the MCMC
+ *                  case); d_times [n_t] is shared as well.
+ *   d_chi2         [n_pv] doubles, overwritten.  A row with bad parameters gets NaN (+ PT_ST_BAD_PARAM).
+ * The sum is formed as the all-out-of-transit value plus, per in-window exposure, the correction
+ * (1-F) w² (2 (o-1) + (1-F)): exposures that cannot be in transit cost one window test and no memory traffic.
+ * Corrections are added with floating-point atomics, so chi2 is reproducible to rounding (~1e-16 relative), not bitwise. */
+int pt_ma_quad_chi2(const pt_table* table, const double* d_times, int64_t n_t, const double* d_params, int64_t n_pv,
+                    int32_t n_pb, int32_t n_ss, double t_exp, const double* d_obs, const double* d_isig, double* d_chi2,
+                    int32_t* d_status, void* stream);
+
 /* Host-buffer convenience forms (the end-to-end path of P:L173/P:L198: copy inputs to the GPU, evaluate, copy the
  * flux back).  All pointers are HOST pointers (pinned memory makes the copies asynchronous); the call allocates
  * stream-ordered scratch on the current device, enqueues H2D copies, the same kernels as above and the D2H copy on an

@@ -157,3 +157,24 @@ def ma_quad_interp(table, k_min, dk, dz, times, params, n_pb: int = 1, n_ss: int
                                   C.c_int32(n_ss), C.c_double(t_exp), _p(f))
     assert rc == 0, rc
     return f
+
+
+def chi2_of_flux(flux, obs, isig):
+    """chi2[pv] = sum_{j,t} ((obs[j][t] - flux[pv][j][t]) * isig[j][t])^2 — the definition (the likelihood the
+    paper proposes to evaluate on the GPU next to z), summed in extended precision over passbands and exposures."""
+    flux = np.asarray(flux, dtype=np.longdouble)
+    o = np.asarray(obs, dtype=np.longdouble).reshape(flux.shape[1:])
+    w = np.asarray(isig, dtype=np.longdouble).reshape(flux.shape[1:])
+    d = (o[None] - flux) * w[None]
+    return np.asarray((d * d).sum(axis=(1, 2)), dtype=np.float64)
+
+
+def ma_quad_chi2(times, params, obs, isig, n_pb: int = 1, n_ss: int = 1, t_exp: float = 0.0, table=None,
+                 prec: str = "f128"):
+    """Fused-likelihood oracle: the exact (table is None) or interpolated flux of this module, then chi2_of_flux.
+    table = (array, k_min, dk, dz)."""
+    if table is None:
+        f = ma_quad_exact(times, params, n_pb, n_ss, t_exp, prec)
+    else:
+        f = ma_quad_interp(table[0], table[1], table[2], table[3], times, params, n_pb, n_ss, t_exp, prec)
+    return chi2_of_flux(f, obs, isig)

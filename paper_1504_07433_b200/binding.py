@@ -20,7 +20,7 @@ PT_F64, PT_F32 = 0, 1
 PT_ST_BAD_PARAM, PT_ST_K_OUT_OF_TABLE = 1, 2
 _ERR = {1: "PT_ERR_NULL", 2: "PT_ERR_SIZE", 3: "PT_ERR_DTYPE", 4: "PT_ERR_TABLE", 5: "PT_ERR_CUDA"}
 
-EXPORTS = ("pt_build_arch", "pt_orbit_z", "pt_ma_quad_exact", "pt_ma_table_build", "pt_ma_quad_interp",
+EXPORTS = ("pt_build_arch", "pt_orbit_z", "pt_ma_quad_exact", "pt_ma_table_build", "pt_ma_quad_interp", "pt_ma_quad_chi2",
            "pt_ma_quad_exact_host", "pt_ma_quad_interp_host", "pt_probe_dfma", "pt_launch_count")
 
 
@@ -52,6 +52,7 @@ def lib() -> C.CDLL:
         L.pt_ma_quad_exact.argtypes = common + [i32, ptr, ptr, ptr]
         L.pt_ma_table_build.argtypes = [dbl, dbl, i32, dbl, i32, i32, i32, ptr, ptr]
         L.pt_ma_quad_interp.argtypes = [C.POINTER(pt_table)] + common + [i32, ptr, ptr, ptr]
+        L.pt_ma_quad_chi2.argtypes = [C.POINTER(pt_table), ptr, i64, ptr, i64, i32, i32, dbl, ptr, ptr, ptr, ptr, ptr]
         L.pt_ma_quad_exact_host.argtypes = common + [i32, ptr, ptr]
         L.pt_ma_quad_interp_host.argtypes = [C.POINTER(pt_table)] + common + [i32, ptr, ptr]
         L.pt_probe_dfma.argtypes = [i32, i32, ptr, ptr]
@@ -155,6 +156,25 @@ def pt_ma_quad_interp(table: Table, times: torch.Tensor, params: torch.Tensor, n
     _check(lib().pt_ma_quad_interp(C.byref(table.desc), times.data_ptr(), n_t, stride, params.data_ptr(), n_pv, n_pb,
                                    n_ss, float(t_exp), _dtype_code(out.dtype), out.data_ptr(),
                                    status.data_ptr() if status is not None else None, _stream()), "pt_ma_quad_interp")
+    return out
+
+
+def pt_ma_quad_chi2(times: torch.Tensor, params: torch.Tensor, obs: torch.Tensor, isig: torch.Tensor, n_pb: int = 1,
+                    n_ss: int = 1, t_exp: float = 0.0, table: Optional[Table] = None, out: Optional[torch.Tensor] = None,
+                    status: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """Fused likelihood chi2[n_pv] against one data set obs/isig [n_pb][n_t] (include/pt.h: pt_ma_quad_chi2)."""
+    times, params, n_pv, n_t, stride = _marshal(times, params, n_pb)
+    if stride != 0:
+        raise PtError("pt_ma_quad_chi2 takes one shared time axis [n_t]")
+    for x in (obs, isig):
+        if not (x.is_cuda and x.dtype == torch.float64 and x.is_contiguous() and x.numel() == n_pb * n_t):
+            raise PtError("obs and isig must be contiguous CUDA float64 tensors of n_pb*n_t elements")
+    if out is None:
+        out = torch.empty(n_pv, dtype=torch.float64, device=times.device)
+    _check(lib().pt_ma_quad_chi2(C.byref(table.desc) if table is not None else None, times.data_ptr(), n_t,
+                                 params.data_ptr(), n_pv, n_pb, n_ss, float(t_exp), obs.data_ptr(), isig.data_ptr(),
+                                 out.data_ptr(), status.data_ptr() if status is not None else None, _stream()),
+           "pt_ma_quad_chi2")
     return out
 
 

@@ -24,6 +24,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <type_traits>
+
 #include "../../include/pt.h"
 #include "pt_basis.cuh"
 #include "pt_orbit.cuh"
@@ -57,6 +59,12 @@ struct FluxArgs {
   double t_exp;
   void* flux;
   int32_t* status;
+  // fused likelihood (OutT = Chi2): observed flux and 1/sigma [n_pb][n_t] shared by all parameter vectors, chi2 [n_pv]
+  const double* obs;
+  const double* isig;
+  double* chi2;
+  const double* base_part;     // partial sums of the all-out-of-transit chi2 (chi2_base_kernel), n_base_part of them
+  int n_base_part;
   // tiling
   int tile_len;            // exposures per tile (multiple of 256, <= kMaxTileLen)
   int tiles_per_pv;
@@ -81,6 +89,7 @@ __device__ __forceinline__ double nan64() { return __longlong_as_double(0x7ff800
 struct PvRec {
   PvConst c;               // orbit constants, k̂, phase window (pt_orbit.cuh)
   const double* tb;        // times of the tile
+  int64_t e0, pv;          // first exposure of the tile in its row; parameter vector (fused likelihood)
   char* ob;                // flux of the tile: row pv, passband 0, first exposure of the tile
   double coef[3];          // single passband: g(1-c)/N, g c/N, g u2/N
   double acc_scale;        // single passband: fixed-point scale of the combined decrement, and its inverse / n_ss
@@ -119,46 +128,78 @@ struct WarpCtr {
   int cur;                      // PvRec of the tile being streamed
 };
 
+// Output tag of the fused likelihood (S§8(f) NEXT-1): no flux is stored; every finished in-window exposure
+// adds its chi2 correction to chi2[pv] instead.
+struct Chi2 { double unused; };
+template <typename OutT> constexpr bool kIsChi2 = std::is_same<OutT, Chi2>::value;
+
 template <typename OutT> struct Vec2;
+template <> struct Vec2<Chi2> { typedef double2 type; };
 template <> struct Vec2<double> { typedef double2 type; };
 template <> struct Vec2<float> { typedef float2 type; };
 
 // flux = 1 for one exposure / an aligned pair of exposures, all passbands (streaming stores: the output is write-once).
 template <bool NPB1, typename OutT>
 __device__ __forceinline__ void store_one(OutT* __restrict__ out, int64_t n_t, int n_pb) {
-  if (NPB1) __stcs(out, (OutT)1.0);
-  else for (int j = 0; j < n_pb; ++j) __stcs(out + (int64_t)j * n_t, (OutT)1.0);
+  if constexpr (kIsChi2<OutT>) {
+    return;   // flux 1 is what the chi2 baseline assumes: nothing to add
+  } else {
+    if (NPB1) __stcs(out, (OutT)1.0);
+    else for (int j = 0; j < n_pb; ++j) __stcs(out + (int64_t)j * n_t, (OutT)1.0);
+  }
 }
 template <bool NPB1, typename OutT>
 __device__ __forceinline__ void store_one_pair(OutT* __restrict__ out, int64_t n_t, int n_pb) {
-  typename Vec2<OutT>::type v;
-  v.x = (OutT)1.0; v.y = (OutT)1.0;
-  if (NPB1) __stcs((typename Vec2<OutT>::type*)out, v);
-  else for (int j = 0; j < n_pb; ++j) __stcs((typename Vec2<OutT>::type*)(out + (int64_t)j * n_t), v);
+  if constexpr (kIsChi2<OutT>) {
+    return;
+  } else {
+    typename Vec2<OutT>::type v;
+    v.x = (OutT)1.0; v.y = (OutT)1.0;
+    if (NPB1) __stcs((typename Vec2<OutT>::type*)out, v);
+    else for (int j = 0; j < n_pb; ++j) __stcs((typename Vec2<OutT>::type*)(out + (int64_t)j * n_t), v);
+  }
+}
+
+// Limb-darkening combine (Eq. 13 with the k-correction of P:L179) of one exposure's mean basis functions, and the
+// stores.  Single passband: the decrement arrives already combined in `le`.
+// One passband's result of a finished exposure: the flux store, or (fused likelihood) the chi2 correction
+//   ((o - F) w)² - ((o - 1) w)² = (1-F) w² (2 (o-1) + (1-F)),   o = observed flux, w = 1/sigma,
+// formed without cancellation from the decrement 1-F.
+template <typename OutT>
+__device__ __forceinline__ void emit(const FluxArgs& A, const PvRec& r, OutT* out, uint32_t e, int j, double dec, double& chi) {
+  if constexpr (kIsChi2<OutT>) {
+    const int64_t idx = (int64_t)j * A.n_t + r.e0 + e;
+    const double o = __ldg(A.obs + idx), w = __ldg(A.isig + idx);
+    chi = fma(dec * w * w, fma(2.0, o - 1.0, dec), chi);
+  } else {
+    __stcs(out + (int64_t)j * A.n_t, (OutT)(1.0 - dec));
+  }
 }
 
 // Limb-darkening combine (Eq. 13 with the k-correction of P:L179) of one exposure's mean basis functions, and the
 // stores.  Single passband: the decrement arrives already combined in `le`.
 template <bool NPB1, typename OutT>
 __device__ __forceinline__ void finish_exposure(const FluxArgs& A, const WarpState& ws, const PvRec& r, uint32_t e,
-                                                double le, double ld, double ed) {
+                                                double le, double ld, double ed, double* chi_acc = nullptr) {
   OutT* out = (OutT*)r.ob + e;
+  double chi = 0.0;
   if (NPB1) {
-    __stcs(out, (OutT)(1.0 - le));
+    emit<OutT>(A, r, out, e, 0, le, chi);
   } else {
     const int n_pb = A.n_pb;
     const int nc = n_pb < kCoefCache ? n_pb : kCoefCache;
-    for (int j = 0; j < nc; ++j) {
-      const double v = 1.0 - fma(ws.coefc[3 * j + 2], ed, fma(ws.coefc[3 * j + 1], ld, ws.coefc[3 * j] * le));
-      __stcs(out + (int64_t)j * A.n_t, (OutT)v);
-    }
+    for (int j = 0; j < nc; ++j)
+      emit<OutT>(A, r, out, e, j, fma(ws.coefc[3 * j + 2], ed, fma(ws.coefc[3 * j + 1], ld, ws.coefc[3 * j] * le)), chi);
     for (int j = nc; j < n_pb; ++j) {   // beyond the cache: coefficients from the parameter row
       const double k = __ldg(r.row + 6 + 3 * j), u1 = __ldg(r.row + 7 + 3 * j), u2 = __ldg(r.row + 8 + 3 * j);
       const double cj = u1 + 2.0 * u2;
       const double gN = k * k * r.ik2 / (1.0 - u1 / 3.0 - u2 / 6.0);
-      const double v = 1.0 - fma(gN * u2, ed, fma(gN * cj, ld, gN * (1.0 - cj) * le));
-      __stcs(out + (int64_t)j * A.n_t, (OutT)v);
+      emit<OutT>(A, r, out, e, j, fma(gN * u2, ed, fma(gN * cj, ld, gN * (1.0 - cj) * le)), chi);
     }
+  }
+  if constexpr (kIsChi2<OutT>) {
+    if (chi_acc) *chi_acc += chi;          // caller sums over the tile (all of it one parameter vector)
+    else atomicAdd(A.chi2 + r.pv, chi);
   }
 }
 
@@ -255,7 +296,9 @@ __device__ __noinline__ void tile_setup(const FluxArgs& A, WarpState& ws, int ri
     }
     if (lane == 0) {
       r.tb = A.times + pv * A.t_stride_pv + e0;
-      r.ob = (char*)A.flux + ((pv * n_pb) * A.n_t + e0) * (int64_t)sizeof(OutT);
+      r.ob = kIsChi2<OutT> ? nullptr : (char*)A.flux + ((pv * n_pb) * A.n_t + e0) * (int64_t)sizeof(OutT);
+      r.e0 = e0;
+      r.pv = pv;
     }
     __syncwarp();
     return;
@@ -278,7 +321,9 @@ __device__ __noinline__ void tile_setup(const FluxArgs& A, WarpState& ws, int ri
   const double ik2 = khat > 1.0e-150 ? rcp_fast(khat * khat) : (khat > 0.0 ? 1.0 / (khat * khat) : 0.0);
   if (lane == 0) {
     r.tb = A.times + pv * A.t_stride_pv + e0;
-    r.ob = (char*)A.flux + ((pv * n_pb) * A.n_t + e0) * (int64_t)sizeof(OutT);
+    r.ob = kIsChi2<OutT> ? nullptr : (char*)A.flux + ((pv * n_pb) * A.n_t + e0) * (int64_t)sizeof(OutT);
+    r.e0 = e0;
+    r.pv = pv;
     r.row = row;
     r.ik2 = ik2;
     r.use_table = 0;
@@ -444,7 +489,8 @@ struct LaneCtx {
 };
 
 template <int MODE, bool NPB1, bool SS1, typename OutT>
-__device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, WarpCtr& C, const LaneCtx& L, int nb, int& ms0, int& msid) {
+__device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, WarpCtr& C, const LaneCtx& L, int nb, int& ms0, int& msid,
+                                        double& chi_acc) {
   const int lane = threadIdx.x & 31;
   const unsigned lt = (1u << lane) - 1u;
   const int cur = C.cur;
@@ -467,8 +513,8 @@ __device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, WarpCt
       const double zs = orbit_z_signed(r.c, fold_phase(t, r.c.t0, r.c.P, r.c.invP, slow_div));
       if (zs >= 0.0 && zs < 1.0 + khat) {
         const Basis b = eval_basis<MODE>(A, r, zs);
-        if (NPB1) finish_exposure<true, OutT>(A, ws, r, e, fma(r.coef[2], b.ed, fma(r.coef[1], b.ld, r.coef[0] * b.le)), 0.0, 0.0);
-        else finish_exposure<false, OutT>(A, ws, r, e, b.le, b.ld, b.ed);
+        if (NPB1) finish_exposure<true, OutT>(A, ws, r, e, fma(r.coef[2], b.ed, fma(r.coef[1], b.ld, r.coef[0] * b.le)), 0.0, 0.0, &chi_acc);
+        else finish_exposure<false, OutT>(A, ws, r, e, b.le, b.ld, b.ed, &chi_acc);
       } else {
         store_one<NPB1, OutT>(ob + e, A.n_t, n_pb);
       }
@@ -641,6 +687,7 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
   bool drain_all = false;        // empty the item queue (ragged last round) before going on
   int keep = EPW;                // z-rounds run while the exposure ring holds at least this many entries
   int ms0 = 0, msid = -1;        // n_ss > 32: sub-round state of the exposure being expanded
+  double chi_acc = 0.0;          // fused likelihood, n_ss == 1: this lane's chi2 corrections of the current tile
   uint32_t base = 0, n_e = 0;
   unsigned long long fetched = 0;
   const double* __restrict__ tb = nullptr;
@@ -659,7 +706,7 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
     {
       const int qc = C.qcount;
       if (qc >= keep) {
-        expand<MODE, NPB1, SS1, OutT>(A, ws, C, L, min(qc, EPW), ms0, msid);
+        expand<MODE, NPB1, SS1, OutT>(A, ws, C, L, min(qc, EPW), ms0, msid, chi_acc);
         continue;
       }
     }
@@ -668,6 +715,12 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
         // tile finished (the exposure ring is empty: keep was 1).  Multi-passband: the coefficient cache belongs to this
         // parameter vector, so the item queue is emptied too.
         if (!NPB1 && !SS1 && C.icount > 0) { drain_all = true; continue; }
+        if (kIsChi2<OutT> && SS1) {   // one atomic per tile: lane sums, then a shuffle tree
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) chi_acc += __shfl_xor_sync(0xffffffffu, chi_acc, o);
+          if (lane == 0 && chi_acc != 0.0) atomicAdd(A.chi2 + pv_cur, chi_acc);
+          chi_acc = 0.0;
+        }
         const unsigned long long nf = __shfl_sync(0xffffffffu, fetched, 0);
         if (!A.per_pv) {
           const int64_t tile = nw + (int64_t)nf;
@@ -769,10 +822,21 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
       base = 0;
       keep = EPW;
       if (r.c.flags & PV_BAD) {
-        for (int j = 0; j < n_pb; ++j)
-          for (uint32_t e = lane; e < n_e; e += 32) ob[(int64_t)j * A.n_t + e] = (OutT)nan64();
+        if constexpr (kIsChi2<OutT>) {
+          if (chunk_cur == 0 && lane == 0) atomicAdd(A.chi2 + pv_cur, nan64());
+        } else {
+          for (int j = 0; j < n_pb; ++j)
+            for (uint32_t e = lane; e < n_e; e += 32) ob[(int64_t)j * A.n_t + e] = (OutT)nan64();
+        }
         base = n_e;       // nothing to stream
         keep = 1;
+      } else if (kIsChi2<OutT> && chunk_cur == 0) {
+        // chi2 of this parameter vector starts from the all-out-of-transit value: partial sums in fixed order
+        double b = 0.0;
+        for (int i = lane; i < A.n_base_part; i += 32) b += A.base_part[i];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) b += __shfl_xor_sync(0xffffffffu, b, o);
+        if (lane == 0) atomicAdd(A.chi2 + pv_cur, b);
       }
       w_invP = r.c.invP; w_c0 = r.w_c0; w_half = r.w_half;
       phase = PH_STREAM;

@@ -93,6 +93,31 @@ __global__ void __launch_bounds__(kThreads) table_kernel(double k_min, double dk
   }
 }
 
+// Fused likelihood, step 1: chi2 of the all-out-of-transit model, sum over (passband, exposure) of ((obs - 1) / sigma)².
+// Block b reduces a contiguous range in a fixed order (strided per-thread sums, then a shared-memory tree) and writes one
+// partial; the flux kernel adds the partials, again in a fixed order, to every parameter vector.  Also zeroes chi2[].
+constexpr int kBaseBlocks = 128;
+__global__ void __launch_bounds__(kThreads) chi2_base_kernel(const double* __restrict__ obs, const double* __restrict__ isig,
+                                                             int64_t n, double* __restrict__ part, double* __restrict__ chi2,
+                                                             int64_t n_pv) {
+  __shared__ double s_sum[kThreads];
+  const int64_t per = (n + gridDim.x - 1) / gridDim.x;
+  const int64_t lo = (int64_t)blockIdx.x * per, hi = min(lo + per, n);
+  double acc = 0.0;
+  for (int64_t i = lo + threadIdx.x; i < hi; i += kThreads) {
+    const double d = (__ldg(obs + i) - 1.0) * __ldg(isig + i);
+    acc = fma(d, d, acc);
+  }
+  s_sum[threadIdx.x] = acc;
+  __syncthreads();
+  for (int o = kThreads / 2; o > 0; o >>= 1) {
+    if (threadIdx.x < o) s_sum[threadIdx.x] += s_sum[threadIdx.x + o];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) part[blockIdx.x] = s_sum[0];
+  for (int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x; i < n_pv; i += (int64_t)gridDim.x * kThreads) chi2[i] = 0.0;
+}
+
 // FP64-pipe peak probe: 8 independent DFMA chains per thread.
 __global__ void __launch_bounds__(kThreads) dfma_probe_kernel(int iters, double* __restrict__ sink) {
   double a0 = threadIdx.x * 1e-3, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
@@ -127,12 +152,18 @@ static int sm_count() {
   return n;
 }
 
+struct Chi2Args {
+  const double* obs;
+  const double* isig;
+};
+constexpr int kDtypeChi2 = 2;   // internal: d_flux is chi2[n_pv], `like` holds the observations
+
 static int launch_flux(int mode, const pt_table* tb, const double* d_times, int64_t n_t, int64_t t_stride_pv,
                        const double* d_params, int64_t n_pv, int n_pb, int n_ss, double t_exp, int dtype, void* d_flux,
-                       int32_t* d_status, cudaStream_t st) {
+                       int32_t* d_status, cudaStream_t st, const Chi2Args* like = nullptr) {
   int rc = check_common(d_times, d_params, d_flux, n_t, t_stride_pv, n_pv, n_pb, n_ss);
   if (rc) return rc;
-  if (dtype != PT_F64 && dtype != PT_F32) return PT_ERR_DTYPE;
+  if (dtype != PT_F64 && dtype != PT_F32 && !(dtype == kDtypeChi2 && like)) return PT_ERR_DTYPE;
   FluxArgs A{};
   A.times = d_times; A.n_t = n_t; A.t_stride_pv = t_stride_pv; A.params = d_params; A.n_pv = n_pv;
   A.n_pb = n_pb; A.n_ss = n_ss; A.t_exp = t_exp; A.flux = d_flux; A.status = d_status;
@@ -155,7 +186,7 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   const int64_t tpp = (n_t + tl - 1) / tl;
   if (tpp > 0x7fffffff || (double)tpp * (double)n_pv > 9.0e18) return PT_ERR_SIZE;
   A.tile_len = (int)tl; A.tiles_per_pv = (int)tpp; A.n_tiles = n_pv * tpp;
-  A.per_pv = (n_pv <= kSchedWords - 2 && tpp >= 2) ? 1 : 0;
+  A.per_pv = (n_pv <= kSchedWords - 2 - kBaseBlocks && tpp >= 2) ? 1 : 0;   // the slot's tail holds the chi2 partials
   int lg = 0;
   while (((int64_t)1 << lg) < (int64_t)n_ss) ++lg;
   A.fx_bits = 61 - lg;
@@ -167,9 +198,20 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   const dim3 grid((unsigned)blocks);
   A.sched = sched_slot();
   if (!A.sched) return PT_ERR_CUDA;
+  if (dtype == kDtypeChi2) {
+    // step 1 of the fused likelihood: out-of-transit baseline into the tail of the scheduler slot, chi2[] zeroed
+    double* part = reinterpret_cast<double*>(A.sched + kSchedWords - kBaseBlocks);
+    const int64_t n_obs = (int64_t)n_pb * n_t;
+    int nb = (int)((n_obs + 4095) / 4096);
+    if (nb > kBaseBlocks) nb = kBaseBlocks;
+    if (nb < 1) nb = 1;
+    chi2_base_kernel<<<nb, kThreads, 0, st>>>(like->obs, like->isig, n_obs, part, (double*)d_flux, n_pv);
+    A.obs = like->obs; A.isig = like->isig; A.chi2 = (double*)d_flux; A.base_part = part; A.n_base_part = nb;
+    A.flux = nullptr;
+  }
   // 16-byte loads/stores need even row lengths/strides and 16-byte aligned bases
   const bool v2 = (n_t % 2 == 0) && (t_stride_pv % 2 == 0) && (reinterpret_cast<uintptr_t>(d_times) % 16 == 0) &&
-                  (reinterpret_cast<uintptr_t>(d_flux) % 16 == 0);
+                  (dtype == kDtypeChi2 || reinterpret_cast<uintptr_t>(d_flux) % 16 == 0);
   const bool p1 = (n_pb == 1), s1 = (n_ss == 1);
 #define PT_LAUNCH(M, VV, P, S, T) flux_kernel<M, VV, P, S, T><<<grid, kThreads, 0, st>>>(A)
 #define PT_LAUNCH_S(M, VV, P, T)                             \
@@ -185,9 +227,9 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
     else PT_LAUNCH_S(M, 1, false, T);                        \
   } while (0)
   if (mode == 0) {
-    if (dtype == PT_F64) PT_LAUNCH_T(0, double); else PT_LAUNCH_T(0, float);
+    if (dtype == PT_F64) PT_LAUNCH_T(0, double); else if (dtype == PT_F32) PT_LAUNCH_T(0, float); else PT_LAUNCH_T(0, Chi2);
   } else {
-    if (dtype == PT_F64) PT_LAUNCH_T(1, double); else PT_LAUNCH_T(1, float);
+    if (dtype == PT_F64) PT_LAUNCH_T(1, double); else if (dtype == PT_F32) PT_LAUNCH_T(1, float); else PT_LAUNCH_T(1, Chi2);
   }
 #undef PT_LAUNCH_T
 #undef PT_LAUNCH_S
@@ -267,6 +309,15 @@ int pt_ma_quad_interp(const pt_table* table, const double* d_times, int64_t n_t,
                      (cudaStream_t)stream);
 }
 
+int pt_ma_quad_chi2(const pt_table* table, const double* d_times, int64_t n_t, const double* d_params, int64_t n_pv,
+                    int32_t n_pb, int32_t n_ss, double t_exp, const double* d_obs, const double* d_isig, double* d_chi2,
+                    int32_t* d_status, void* stream) {
+  if (!d_obs || !d_isig) return PT_ERR_NULL;
+  const Chi2Args like{d_obs, d_isig};
+  return launch_flux(table ? 1 : 0, table, d_times, n_t, 0, d_params, n_pv, n_pb, n_ss, t_exp, kDtypeChi2, d_chi2, d_status,
+                     (cudaStream_t)stream, &like);
+}
+
 // ---- host-buffer forms: H2D, kernels, D2H on an internal stream, then wait.
 static int run_host(int mode, const pt_table* tb, const double* h_times, int64_t n_t, int64_t t_stride_pv,
                     const double* h_params, int64_t n_pv, int n_pb, int n_ss, double t_exp, int dtype, void* h_flux,
@@ -275,7 +326,16 @@ static int run_host(int mode, const pt_table* tb, const double* h_times, int64_t
   if (rc) return rc;
   if (dtype != PT_F64 && dtype != PT_F32) return PT_ERR_DTYPE;
   static thread_local cudaStream_t st = nullptr;
-  if (!st && cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) != cudaSuccess) return PT_ERR_CUDA;
+  if (!st) {
+    if (cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) != cudaSuccess) return PT_ERR_CUDA;
+    // keep the stream-ordered scratch in the pool between calls (the default hands it back at every synchronisation)
+    int dev = 0;
+    cudaMemPool_t pool;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+      uint64_t keep = UINT64_MAX;
+      cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    }
+  }
   const size_t nb_t = sizeof(double) * (size_t)(t_stride_pv == 0 ? n_t : (n_pv - 1) * t_stride_pv + n_t);
   const size_t nb_p = sizeof(double) * (size_t)n_pv * (6 + 3 * (size_t)n_pb);
   const size_t nb_f = (dtype == PT_F64 ? 8 : 4) * (size_t)n_pv * n_pb * n_t;

@@ -365,3 +365,58 @@ def test_concurrent_streams(pt, oracle):
     for fa, fb in outs:
         assert np.abs(fa.cpu().numpy() - ra).max() <= TOL64
         assert np.abs(fb.cpu().numpy() - rb).max() <= TOL64
+
+
+# ------------------------------------------------------------------------------------------- fused likelihood (NEXT-1)
+def _data_for(oracle, w, truth_row=0, sigma=2e-4, seed=3):
+    """Synthetic observations: the oracle's flux of one parameter vector plus seeded Gaussian noise."""
+    wt = inputs.Workload("truth", w.times, w.params[truth_row:truth_row + 1], w.n_pb, w.n_ss, w.t_exp)
+    f = ora_exact(oracle, wt, "f64")[0]
+    rng = np.random.default_rng(seed)
+    obs = f + sigma * rng.standard_normal(f.shape)
+    isig = np.full(f.shape, 1.0 / sigma) * rng.uniform(0.5, 2.0, f.shape)
+    return obs, isig
+
+
+@pytest.mark.parametrize("cfg", ["c2", "c2_ss1", "c3", "short", "ecc"])
+def test_chi2_exact_parity(pt, oracle, cfg):
+    if cfg == "c2":
+        w = inputs.config2(n_pv=24, n_t=9000)
+    elif cfg == "c2_ss1":
+        w = inputs.config2(n_pv=24, n_t=9001); w.n_ss = 1
+    elif cfg == "c3":
+        w = inputs.config3(n_pv=64, n_pb=5, n_t=601)
+    elif cfg == "short":
+        w = inputs.config3(n_pv=1500, n_pb=2, n_t=40); w.n_ss, w.t_exp = 3, 0.003
+    else:
+        wd = inputs.dense_transit(n_pv=1, n_t=2000)
+        rng = np.random.default_rng(9)
+        p = np.repeat(wd.params, 200, 0)
+        p[:, 6] *= rng.uniform(0.9, 1.1, 200); p[:, 0] += rng.normal(0, 2e-3, 200); p[:, 4] = rng.uniform(0.0, 0.5, 200)
+        w = inputs.Workload("ecc", wd.times[0].copy(), p)
+    obs, isig = _data_for(oracle, w)
+    st = torch.zeros(2, dtype=torch.int32, device="cuda")
+    c = pt.pt_ma_quad_chi2(dev(w.times), dev(w.params), dev(obs), dev(isig), w.n_pb, w.n_ss, w.t_exp, status=st)
+    r = oracle.ma_quad_chi2(w.times, w.params, obs, isig, w.n_pb, w.n_ss, w.t_exp)
+    assert st.cpu().tolist() == [0, 0]
+    # flux parity is 1e-12 abs; a residual of r sigma turns that into 2 r 1e-12/sigma per term: relative 1e-10 is ample
+    assert np.abs(c.cpu().numpy() - r).max() <= 1e-10 * np.abs(r).max(), (np.abs(c.cpu().numpy() - r).max(), np.abs(r).max())
+    # and it is the same number as the library's own flux pushed through the definition
+    f = gpu_exact(pt, w)
+    assert np.allclose(c.cpu().numpy(), oracle.chi2_of_flux(f, obs, isig), rtol=1e-11)
+
+
+def test_chi2_interp_and_bad_rows(pt, oracle):
+    c4 = dict(k_min=0.05, k_max=0.25, n_k=41, z_max=1.25, n_z=1251)
+    tb = pt.pt_ma_table_build(dtype=torch.float32, n_fn=4, **c4)
+    w = inputs.config4(n_pv=40, n_t=6000)
+    w.params[3, 6] = 0.31          # off the table: exact fallback
+    w.params[7, 1] = -2.0          # bad period: NaN
+    obs, isig = _data_for(oracle, w)
+    st = torch.zeros(2, dtype=torch.int32, device="cuda")
+    c = pt.pt_ma_quad_chi2(dev(w.times), dev(w.params), dev(obs), dev(isig), table=tb, status=st).cpu().numpy()
+    r = oracle.ma_quad_chi2(w.times, w.params, obs, isig, table=(tb.data.cpu().numpy(), tb.k_min, tb.dk, tb.dz))
+    assert np.isnan(c[7]) and np.isnan(r[7])
+    ok = np.arange(40) != 7
+    assert np.abs(c[ok] - r[ok]).max() <= 1e-10 * np.abs(r[ok]).max()
+    assert st.cpu().tolist() == [pt.PT_ST_BAD_PARAM | pt.PT_ST_K_OUT_OF_TABLE, 2]

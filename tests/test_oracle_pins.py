@@ -368,3 +368,31 @@ def test_f64_vs_f128_flux_on_bulk_workloads(oracle):
     a = oracle.ma_quad_exact(w.times, w.params, n_ss=3, t_exp=w.t_exp, prec="f64")
     b = oracle.ma_quad_exact(w.times, w.params, n_ss=3, t_exp=w.t_exp, prec="f128")
     assert np.abs(a - b).max() <= 1e-11
+
+
+# ------------------------------------------------------------------------------------------- likelihood (S§8(f) NEXT-1)
+def test_chi2_definition_pins(oracle):
+    """chi2_of_flux against facts that do not involve it: zero residuals, one known residual, scaling with 1/sigma,
+    additivity over passbands, and the expectation n for unit-variance noise."""
+    w = inputs.config3(n_pv=3, n_pb=2, n_t=200)
+    f = oracle.ma_quad_exact(w.times, w.params, 2, 1, 0.0, prec="f64")
+    ones = np.ones((2, 200))
+    assert np.all(oracle.chi2_of_flux(f, f[1], 7.0 * ones)[1] == 0.0)
+    obs = f[0].copy()
+    obs[1, 17] += 3e-4                                        # one residual of 3 sigma at sigma = 1e-4
+    c = oracle.chi2_of_flux(f[:1], obs, 1e4 * ones)
+    assert abs(c[0] - 9.0) < 1e-9
+    assert np.allclose(oracle.chi2_of_flux(f, obs, 2e4 * ones), 4.0 * oracle.chi2_of_flux(f, obs, 1e4 * ones), rtol=1e-14)
+    both = oracle.chi2_of_flux(f, obs, 1e4 * ones)
+    each = sum(oracle.chi2_of_flux(f[:, j:j + 1], obs[j:j + 1], 1e4 * ones[j:j + 1]) for j in range(2))
+    assert np.allclose(both, each, rtol=1e-14)
+    rng = np.random.default_rng(5)
+    sig = 2e-4
+    noisy = f[2] + sig * rng.standard_normal(f[2].shape)
+    c = oracle.chi2_of_flux(f[2:3], noisy, ones / sig)[0]
+    assert abs(c - 400.0) < 5 * np.sqrt(2 * 400.0)              # chi-square with 400 degrees of freedom
+    # the decomposition the kernel uses is an identity: ((o-F)w)^2 = ((o-1)w)^2 + (1-F) w^2 (2(o-1) + (1-F))
+    o, F, ww = noisy, f[2], ones / sig
+    lhs = ((o - F) * ww) ** 2
+    rhs = ((o - 1) * ww) ** 2 + (1 - F) * ww ** 2 * (2 * (o - 1) + (1 - F))
+    assert np.abs(lhs - rhs).max() <= 1e-9 * max(1.0, np.abs(lhs).max())
