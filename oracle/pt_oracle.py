@@ -178,3 +178,14 @@ def ma_quad_chi2(times, params, obs, isig, n_pb: int = 1, n_ss: int = 1, t_exp: 
     else:
         f = ma_quad_interp(table[0], table[1], table[2], table[3], times, params, n_pb, n_ss, t_exp, prec)
     return chi2_of_flux(f, obs, isig)
+
+
+def ma_quad_exact_pbk(times, params, n_pb: int = 1, n_ss: int = 1, t_exp: float = 0.0, prec: str = "f128"):
+    """Exact per-passband-k model (what the mean-k evaluation of P:L179 approximates): passband j is the
+    single-passband model of the row [t0, P, a, i, e, w, k_j, u1_j, u2_j]."""
+    params = np.atleast_2d(np.asarray(params, dtype=np.float64))
+    out = []
+    for j in range(n_pb):
+        row = np.concatenate([params[:, :6], params[:, 6 + 3 * j:9 + 3 * j]], axis=1)
+        out.append(ma_quad_exact(times, row, 1, n_ss, t_exp, prec)[:, 0])
+    return np.stack(out, axis=1)

@@ -20,7 +20,7 @@ PT_F64, PT_F32 = 0, 1
 PT_ST_BAD_PARAM, PT_ST_K_OUT_OF_TABLE = 1, 2
 _ERR = {1: "PT_ERR_NULL", 2: "PT_ERR_SIZE", 3: "PT_ERR_DTYPE", 4: "PT_ERR_TABLE", 5: "PT_ERR_CUDA"}
 
-EXPORTS = ("pt_build_arch", "pt_orbit_z", "pt_ma_quad_exact", "pt_ma_table_build", "pt_ma_quad_interp", "pt_ma_quad_chi2",
+EXPORTS = ("pt_build_arch", "pt_orbit_z", "pt_ma_quad_exact", "pt_ma_table_build", "pt_ma_quad_interp", "pt_ma_quad_chi2", "pt_ma_quad_exact_pbk",
            "pt_ma_quad_exact_host", "pt_ma_quad_interp_host", "pt_probe_dfma", "pt_launch_count")
 
 
@@ -50,6 +50,7 @@ def lib() -> C.CDLL:
         L.pt_launch_count.restype = i64
         L.pt_orbit_z.argtypes = common + [ptr, ptr]
         L.pt_ma_quad_exact.argtypes = common + [i32, ptr, ptr, ptr]
+        L.pt_ma_quad_exact_pbk.argtypes = common + [i32, ptr, ptr, ptr]
         L.pt_ma_table_build.argtypes = [dbl, dbl, i32, dbl, i32, i32, i32, ptr, ptr]
         L.pt_ma_quad_interp.argtypes = [C.POINTER(pt_table)] + common + [i32, ptr, ptr, ptr]
         L.pt_ma_quad_chi2.argtypes = [C.POINTER(pt_table), ptr, i64, ptr, i64, i32, i32, dbl, ptr, ptr, ptr, ptr, ptr]
@@ -123,6 +124,20 @@ def pt_ma_quad_exact(times: torch.Tensor, params: torch.Tensor, n_pb: int = 1, n
     _check(lib().pt_ma_quad_exact(times.data_ptr(), n_t, stride, params.data_ptr(), n_pv, n_pb, n_ss, float(t_exp),
                                   _dtype_code(out.dtype), out.data_ptr(),
                                   status.data_ptr() if status is not None else None, _stream()), "pt_ma_quad_exact")
+    return out
+
+
+def pt_ma_quad_exact_pbk(times: torch.Tensor, params: torch.Tensor, n_pb: int = 1, n_ss: int = 1, t_exp: float = 0.0,
+                         dtype: torch.dtype = torch.float64, out: Optional[torch.Tensor] = None,
+                         status: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """Exact flux with every passband at its own radius ratio (include/pt.h: pt_ma_quad_exact_pbk)."""
+    times, params, n_pv, n_t, stride = _marshal(times, params, n_pb)
+    if out is None:
+        out = torch.empty((n_pv, n_pb, n_t), dtype=dtype, device=times.device)
+    _check(lib().pt_ma_quad_exact_pbk(times.data_ptr(), n_t, stride, params.data_ptr(), n_pv, n_pb, n_ss, float(t_exp),
+                                      _dtype_code(out.dtype), out.data_ptr(),
+                                      status.data_ptr() if status is not None else None, _stream()),
+           "pt_ma_quad_exact_pbk")
     return out
 
 

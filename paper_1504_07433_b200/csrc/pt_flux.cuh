@@ -59,6 +59,11 @@ struct FluxArgs {
   double t_exp;
   void* flux;
   int32_t* status;
+  // views (exact per-passband-k mode launches the single-passband kernel once per passband of a wider row)
+  int64_t row_stride;          // doubles per parameter row
+  int pb_first;                // first passband of the row this launch looks at
+  int64_t flux_pv_stride;      // flux elements between parameter vectors
+  int64_t flux_off;            // flux element offset of this launch's first passband
   // fused likelihood (OutT = Chi2): observed flux and 1/sigma [n_pb][n_t] shared by all parameter vectors, chi2 [n_pv]
   const double* obs;
   const double* isig;
@@ -296,18 +301,19 @@ __device__ __noinline__ void tile_setup(const FluxArgs& A, WarpState& ws, int ri
     }
     if (lane == 0) {
       r.tb = A.times + pv * A.t_stride_pv + e0;
-      r.ob = kIsChi2<OutT> ? nullptr : (char*)A.flux + ((pv * n_pb) * A.n_t + e0) * (int64_t)sizeof(OutT);
+      r.ob = kIsChi2<OutT> ? nullptr : (char*)A.flux + (pv * A.flux_pv_stride + A.flux_off + e0) * (int64_t)sizeof(OutT);
       r.e0 = e0;
       r.pv = pv;
     }
     __syncwarp();
     return;
   }
-  const double* row = A.params + pv * (6 + 3 * (int64_t)n_pb);
+  const double* row = A.params + pv * A.row_stride;
+  const double* pbp = row + 6 + 3 * A.pb_first;   // this launch's passbands: (k, u1, u2) triples
   bool ok = true;
   double ksum = 0.0, N0 = 1.0;
   for (int j = 0; j < n_pb; ++j) {
-    const double k = __ldg(row + 6 + 3 * j), u1 = __ldg(row + 7 + 3 * j), u2 = __ldg(row + 8 + 3 * j);
+    const double k = __ldg(pbp + 3 * j), u1 = __ldg(pbp + 3 * j + 1), u2 = __ldg(pbp + 3 * j + 2);
     const double N = 1.0 - u1 / 3.0 - u2 / 6.0;
     if (!(isfinite(k) && isfinite(u1) && isfinite(u2)) || !(k >= 0.0) || N == 0.0) ok = false;
     ksum += k;
@@ -321,7 +327,7 @@ __device__ __noinline__ void tile_setup(const FluxArgs& A, WarpState& ws, int ri
   const double ik2 = khat > 1.0e-150 ? rcp_fast(khat * khat) : (khat > 0.0 ? 1.0 / (khat * khat) : 0.0);
   if (lane == 0) {
     r.tb = A.times + pv * A.t_stride_pv + e0;
-    r.ob = kIsChi2<OutT> ? nullptr : (char*)A.flux + ((pv * n_pb) * A.n_t + e0) * (int64_t)sizeof(OutT);
+    r.ob = kIsChi2<OutT> ? nullptr : (char*)A.flux + (pv * A.flux_pv_stride + A.flux_off + e0) * (int64_t)sizeof(OutT);
     r.e0 = e0;
     r.pv = pv;
     r.row = row;
@@ -337,7 +343,7 @@ __device__ __noinline__ void tile_setup(const FluxArgs& A, WarpState& ws, int ri
     return;
   }
   if (NPB1) {
-    const double u1 = __ldg(row + 7), u2 = __ldg(row + 8);
+    const double u1 = __ldg(pbp + 1), u2 = __ldg(pbp + 2);
     const double cj = u1 + 2.0 * u2;
     const double gN = 1.0 / N0;                           // k²/k̂² = 1 for a single passband
     const double c0 = gN * (1.0 - cj), c1 = gN * cj, c2 = gN * u2;
@@ -352,7 +358,7 @@ __device__ __noinline__ void tile_setup(const FluxArgs& A, WarpState& ws, int ri
     }
   } else {
     for (int j = lane; j < n_pb && j < kCoefCache; j += 32) {
-      const double k = __ldg(row + 6 + 3 * j), u1 = __ldg(row + 7 + 3 * j), u2 = __ldg(row + 8 + 3 * j);
+      const double k = __ldg(pbp + 3 * j), u1 = __ldg(pbp + 3 * j + 1), u2 = __ldg(pbp + 3 * j + 2);
       const double cj = u1 + 2.0 * u2;
       const double gN = k * k * ik2 / (1.0 - u1 / 3.0 - u2 / 6.0);
       ws.coefc[3 * j + 0] = gN * (1.0 - cj);

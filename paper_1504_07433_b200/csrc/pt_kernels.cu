@@ -160,13 +160,18 @@ constexpr int kDtypeChi2 = 2;   // internal: d_flux is chi2[n_pv], `like` holds 
 
 static int launch_flux(int mode, const pt_table* tb, const double* d_times, int64_t n_t, int64_t t_stride_pv,
                        const double* d_params, int64_t n_pv, int n_pb, int n_ss, double t_exp, int dtype, void* d_flux,
-                       int32_t* d_status, cudaStream_t st, const Chi2Args* like = nullptr) {
+                       int32_t* d_status, cudaStream_t st, const Chi2Args* like = nullptr, int pb_view = -1, int n_pb_row = 0) {
   int rc = check_common(d_times, d_params, d_flux, n_t, t_stride_pv, n_pv, n_pb, n_ss);
   if (rc) return rc;
   if (dtype != PT_F64 && dtype != PT_F32 && !(dtype == kDtypeChi2 && like)) return PT_ERR_DTYPE;
   FluxArgs A{};
   A.times = d_times; A.n_t = n_t; A.t_stride_pv = t_stride_pv; A.params = d_params; A.n_pv = n_pv;
   A.n_pb = n_pb; A.n_ss = n_ss; A.t_exp = t_exp; A.flux = d_flux; A.status = d_status;
+  A.row_stride = 6 + 3 * (int64_t)n_pb; A.pb_first = 0; A.flux_pv_stride = (int64_t)n_pb * n_t; A.flux_off = 0;
+  if (pb_view >= 0) {   // single-passband view of passband `pb_view` in rows of n_pb_row passbands
+    A.row_stride = 6 + 3 * (int64_t)n_pb_row; A.pb_first = pb_view;
+    A.flux_pv_stride = (int64_t)n_pb_row * n_t; A.flux_off = (int64_t)pb_view * n_t;
+  }
   if (mode == 1) {
     if (!tb || !tb->d_data || tb->n_k < 2 || tb->n_z < 2 || (tb->n_fn != 3 && tb->n_fn != 4) || !(tb->dk > 0.0) ||
         !(tb->dz > 0.0) || (tb->dtype != PT_F64 && tb->dtype != PT_F32))
@@ -282,6 +287,17 @@ int pt_ma_quad_exact(const double* d_times, int64_t n_t, int64_t t_stride_pv, co
                      void* stream) {
   return launch_flux(0, nullptr, d_times, n_t, t_stride_pv, d_params, n_pv, n_pb, n_ss, t_exp, dtype, d_flux, d_status,
                      (cudaStream_t)stream);
+}
+
+int pt_ma_quad_exact_pbk(const double* d_times, int64_t n_t, int64_t t_stride_pv, const double* d_params, int64_t n_pv,
+                         int32_t n_pb, int32_t n_ss, double t_exp, int32_t dtype, void* d_flux, int32_t* d_status,
+                         void* stream) {
+  int rc = check_common(d_times, d_params, d_flux, n_t, t_stride_pv, n_pv, n_pb, n_ss);
+  if (rc) return rc;
+  for (int j = 0; j < n_pb && rc == PT_OK; ++j)
+    rc = launch_flux(0, nullptr, d_times, n_t, t_stride_pv, d_params, n_pv, 1, n_ss, t_exp, dtype, d_flux, d_status,
+                     (cudaStream_t)stream, nullptr, j, n_pb);
+  return rc;
 }
 
 int pt_ma_table_build(double k_min, double k_max, int32_t n_k, double z_max, int32_t n_z, int32_t dtype, int32_t n_fn,

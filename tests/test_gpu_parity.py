@@ -420,3 +420,16 @@ def test_chi2_interp_and_bad_rows(pt, oracle):
     ok = np.arange(40) != 7
     assert np.abs(c[ok] - r[ok]).max() <= 1e-10 * np.abs(r[ok]).max()
     assert st.cpu().tolist() == [pt.PT_ST_BAD_PARAM | pt.PT_ST_K_OUT_OF_TABLE, 2]
+
+
+# ------------------------------------------------------------------------------------------- exact per-passband k (NEXT-2)
+@pytest.mark.parametrize("n_pv,n_pb,n_t,n_ss", [(64, 20, 600, 1), (9, 3, 2501, 4), (200, 2, 33, 1)])
+def test_per_passband_k_mode(pt, oracle, n_pv, n_pb, n_t, n_ss):
+    w = inputs.config3(n_pv=n_pv, n_pb=n_pb, n_t=n_t)
+    w.params[:, 6::3] *= np.linspace(0.7, 1.4, n_pb)[None, :]       # a wide spread of radius ratios
+    w.n_ss, w.t_exp = n_ss, 0.003
+    f = pt.pt_ma_quad_exact_pbk(dev(w.times), dev(w.params), n_pb, n_ss, w.t_exp).cpu().numpy()
+    r = oracle.ma_quad_exact_pbk(w.times, w.params, n_pb, n_ss, w.t_exp)
+    assert np.abs(f - r).max() <= TOL64
+    f32 = pt.pt_ma_quad_exact_pbk(dev(w.times), dev(w.params), n_pb, n_ss, w.t_exp, dtype=torch.float32).cpu().numpy()
+    assert np.abs(f32 - r).max() <= TOL32

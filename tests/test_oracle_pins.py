@@ -396,3 +396,19 @@ def test_chi2_definition_pins(oracle):
     lhs = ((o - F) * ww) ** 2
     rhs = ((o - 1) * ww) ** 2 + (1 - F) * ww ** 2 * (2 * (o - 1) + (1 - F))
     assert np.abs(lhs - rhs).max() <= 1e-9 * max(1.0, np.abs(lhs).max())
+
+
+def test_per_passband_k_mode_pins(oracle):
+    """Exact per-passband-k oracle: equal k in every passband reduces to the mean-k model; with config-3's spread the two
+    differ by the few 1e-4 SURVEY §8(f) quotes; a uniform-disk passband inside the limb is exactly 1 - k_j²."""
+    w = inputs.config3(n_pv=4, n_pb=3, n_t=120)
+    p = w.params.copy()
+    a = oracle.ma_quad_exact_pbk(w.times, p, 3, prec="f64")
+    b = oracle.ma_quad_exact(w.times, p, 3, prec="f64")
+    d = np.abs(a - b).max()
+    assert 1e-6 < d < 2e-3
+    p[:, 9] = p[:, 6]; p[:, 12] = p[:, 6]
+    assert np.abs(oracle.ma_quad_exact_pbk(w.times, p, 3, prec="f64") - oracle.ma_quad_exact(w.times, p, 3, prec="f64")).max() < 1e-14
+    q = np.array([[0.0, 3.0, 8.0, np.pi / 2, 0.0, 0.0, 0.1, 0.0, 0.0, 0.2, 0.0, 0.0]])
+    f = oracle.ma_quad_exact_pbk(np.array([0.0]), q, 2, prec="f64")
+    assert abs(f[0, 0, 0] - (1 - 0.01)) < 1e-15 and abs(f[0, 1, 0] - (1 - 0.04)) < 1e-15
