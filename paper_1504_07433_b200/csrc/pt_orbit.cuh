@@ -113,6 +113,17 @@ __device__ __forceinline__ void kepler_newton(double M, double e, double sin_e, 
 // Signed projected separation at pinned folded phase ph (cycles): +z in front of the star, -z behind.
 __device__ __forceinline__ double orbit_z_signed(const PvConst& c, double ph) {
   if (c.flags & PV_CIRCULAR) {
+    if (fabs(ph) <= 0.125) {
+      // within an eighth of a cycle of conjunction (every transit of a/R* > 1.5): no range reduction, no cosine;
+      // z² = a² (cos²i + sin²i sin²φ), planet in front (cos φ > 0)
+      const double r = kC[C_TWOPI] * ph, r2 = r * r;
+      double ps = kTrig[0];
+#pragma unroll
+      for (int j = 1; j < 7; ++j) ps = fma(ps, r2, kTrig[j]);
+      const double sn = fma(ps * r2, r, r);
+      const double ci2 = c.cosi * c.cosi;
+      return c.a * sqrt_fast(fmax(fma(1.0 - ci2, sn * sn, ci2), 0x1p-1000));
+    }
     double sn, cs;
     sincos_bounded(kC[C_TWOPI] * ph, &sn, &cs);
     const double cc = c.cosi * cs;
