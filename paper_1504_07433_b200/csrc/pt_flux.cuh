@@ -116,12 +116,15 @@ struct Slot {              // a supersampled exposure with subsamples still in t
 
 struct WarpState {
   PvRec pv[kPvRing];
-  Slot slots[kSlots];
-  double item_z[kItemQ];
-  uint16_t item_tag[kItemQ];    // supersampled: slot index; n_ss == 1: tile-local exposure index
-  uint8_t item_ring[kItemQ];    // n_ss == 1: PvRec index
   uint16_t expq[kExpQ];
   double coefc[3 * kCoefCache];
+};
+
+// The supersampled path's part of a warp's shared state (the n_ss == 1 kernels do not allocate it).
+struct SsState {
+  Slot slots[kSlots];
+  double item_z[kItemQ];
+  uint16_t item_tag[kItemQ];    // slot index of the queued subsample
 };
 
 // Ring positions of one warp.  They are warp-uniform and live in registers: every stage is inlined at its single call
@@ -409,31 +412,24 @@ __device__ __forceinline__ bool in_window2(double t, double invP, double c0, dou
 #define PT_BASIS_INLINE __forceinline__
 #endif
 template <int MODE, bool NPB1, bool SS1, typename OutT>
-__device__ PT_BASIS_INLINE void basis_round(const FluxArgs& A, WarpState& ws, WarpCtr& C, int n) {
+__device__ PT_BASIS_INLINE void basis_round(const FluxArgs& A, WarpState& ws, SsState& ss, WarpCtr& C, int n) {
   const int lane = threadIdx.x & 31;
   const bool act = lane < n;
   const int ihead = C.ihead;
   const int idx = (ihead + lane) & (kItemQ - 1);
   if (SS1) {
-    if (act) {
-      const double z = ws.item_z[idx];
-      const uint32_t e = ws.item_tag[idx];
-      const PvRec& r = ws.pv[ws.item_ring[idx]];
-      const Basis b = eval_basis<MODE>(A, r, z);
-      if (NPB1) finish_exposure<true, OutT>(A, ws, r, e, fma(r.coef[2], b.ed, fma(r.coef[1], b.ld, r.coef[0] * b.le)), 0.0, 0.0);
-      else finish_exposure<false, OutT>(A, ws, r, e, b.le, b.ld, b.ed);
-    }
+    return;   // the n_ss == 1 path evaluates its samples in the z-round and never queues items
   } else {
     constexpr int NACC = NPB1 ? 1 : 3;
-    const int sid = act ? (int)ws.item_tag[idx] : -1 - lane;   // inactive lanes: unique ids, never equal to a neighbour's
+    const int sid = act ? (int)ss.item_tag[idx] : -1 - lane;   // inactive lanes: unique ids, never equal to a neighbour's
     long long v[NACC];
 #pragma unroll
     for (int a = 0; a < NACC; ++a) v[a] = 0;
     int ring = 0;
     if (act) {
-      ring = ws.slots[sid].ring;
+      ring = ss.slots[sid].ring;
       const PvRec& r = ws.pv[ring];
-      const Basis b = eval_basis<MODE>(A, r, ws.item_z[idx]);
+      const Basis b = eval_basis<MODE>(A, r, ss.item_z[idx]);
       if (NPB1) {
         v[0] = __double2ll_rn(fma(r.coef[2], b.ed, fma(r.coef[1], b.ld, r.coef[0] * b.le)) * r.acc_scale);
       } else {
@@ -459,7 +455,7 @@ __device__ PT_BASIS_INLINE void basis_round(const FluxArgs& A, WarpState& ws, Wa
     const bool tail = act && (lane == 31 || snext != sid);
     if (tail) {
       const int head = 31 - __clz(heads & (0xffffffffu >> (31 - lane)));
-      Slot& s = ws.slots[sid];
+      Slot& s = ss.slots[sid];
       const int rem = s.remaining - (lane - head + 1);
       if (rem == 0) {
         const PvRec& r = ws.pv[ring];
@@ -495,7 +491,7 @@ struct LaneCtx {
 };
 
 template <int MODE, bool NPB1, bool SS1, typename OutT>
-__device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, WarpCtr& C, const LaneCtx& L, int nb, int& ms0, int& msid,
+__device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, SsState& ss, WarpCtr& C, const LaneCtx& L, int nb, int& ms0, int& msid,
                                         double& chi_acc) {
   const int lane = threadIdx.x & 31;
   const unsigned lt = (1u << lane) - 1u;
@@ -553,7 +549,7 @@ __device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, WarpCt
         nalloc = __popc(hm);
         if (act && g == 0) {
           if (has) {
-            Slot& sl = ws.slots[sid];
+            Slot& sl = ss.slots[sid];
             sl.acc[0] = 0; sl.acc[1] = 0; sl.acc[2] = 0;
             sl.remaining = cnt; sl.e = (uint16_t)e; sl.ring = (uint16_t)cur;
           } else {
@@ -565,18 +561,18 @@ __device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, WarpCt
           sid = C.slot_next & (kSlots - 1);
           nalloc = 1;
           if (lane == 0) {
-            Slot& sl = ws.slots[sid];
+            Slot& sl = ss.slots[sid];
             sl.acc[0] = 0; sl.acc[1] = 0; sl.acc[2] = 0;
             sl.remaining = kRemBias; sl.e = (uint16_t)e; sl.ring = (uint16_t)cur;
           }
           __syncwarp();
         }
-        if (lane == 0) ws.slots[sid].remaining += __popc(m);
+        if (lane == 0) ss.slots[sid].remaining += __popc(m);
       }
       if (p) {
         const int pos = (C.ihead + C.icount + __popc(m & lt)) & (kItemQ - 1);
-        ws.item_z[pos] = zs;
-        ws.item_tag[pos] = (uint16_t)sid;
+        ss.item_z[pos] = zs;
+        ss.item_tag[pos] = (uint16_t)sid;
       }
       __syncwarp();
       C.icount += __popc(m);
@@ -591,7 +587,7 @@ __device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, WarpCt
       if (sid < 0) {
         if (lane == 0) store_one<NPB1, OutT>(ob + e, A.n_t, n_pb);
       } else if (lane == 0) {
-        Slot& sl = ws.slots[sid];
+        Slot& sl = ss.slots[sid];
         const int rem = sl.remaining - kRemBias;
         sl.remaining = rem;
         if (rem == 0) {   // every subsample was already evaluated by the basis rounds in between
@@ -643,6 +639,8 @@ __device__ __forceinline__ bool next_pv(const FluxArgs& A, int64_t& pv, int& chu
 template <int MODE, int V, bool NPB1, bool SS1, typename OutT>
 __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __grid_constant__ FluxArgs A) {
   __shared__ WarpState s_ws[kWarpsPerBlock];
+  __shared__ SsState s_ss[SS1 ? 1 : kWarpsPerBlock];
+  SsState& ss = s_ss[SS1 ? 0 : (threadIdx.x >> 5)];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   WarpState& ws = s_ws[warp];
   WarpCtr C;
@@ -704,7 +702,7 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
     if (!SS1) {
       const int ic = C.icount;
       if (ic >= 32 || (drain_all && ic > 0)) {
-        basis_round<MODE, NPB1, SS1, OutT>(A, ws, C, min(ic, 32));
+        basis_round<MODE, NPB1, SS1, OutT>(A, ws, ss, C, min(ic, 32));
         continue;
       }
       drain_all = false;
@@ -712,7 +710,7 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
     {
       const int qc = C.qcount;
       if (qc >= keep) {
-        expand<MODE, NPB1, SS1, OutT>(A, ws, C, L, min(qc, EPW), ms0, msid, chi_acc);
+        expand<MODE, NPB1, SS1, OutT>(A, ws, ss, C, L, min(qc, EPW), ms0, msid, chi_acc);
         continue;
       }
     }
@@ -812,7 +810,7 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
       const int ring = NPB1 ? ((C.cur + 1) & (kPvRing - 1)) : 0;
       if (!SS1 && C.icount > 0) {
         bool clash = true;
-        if (NPB1) clash = ((int)ws.slots[ws.item_tag[C.ihead]].ring == ring);
+        if (NPB1) clash = ((int)ss.slots[ss.item_tag[C.ihead]].ring == ring);
         if (clash) { drain_all = true; continue; }
       }
       fetched = 0;
