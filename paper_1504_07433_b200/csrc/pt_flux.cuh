@@ -38,8 +38,11 @@ constexpr int kWarpsPerBlock = kThreads / 32;
 #define PT_MIN_BLOCKS 3   // resident blocks per SM the flux kernel is compiled for (register cap 65536/(256*PT_MIN_BLOCKS))
 #endif
 constexpr int kMaxPassbands = 1024;
-constexpr int kUnroll = 4;      // 32-exposure groups a warp streams per iteration (independent loads in flight)
-constexpr int kExpQ = 512;      // exposure ring: >= 32*kUnroll*2 + 32 entries, power of two, uint16 tile-local indices
+#ifndef PT_UNROLL
+#define PT_UNROLL 4
+#endif
+constexpr int kUnroll = PT_UNROLL;      // 32-exposure groups a warp streams per iteration (independent loads in flight)
+constexpr int kExpQ = PT_UNROLL > 4 ? 1024 : 512;      // exposure ring: >= 32*kUnroll*2 + 32 entries, power of two, uint16 tile-local indices
 constexpr int kItemQ = 64;      // item ring: at most 31 left over + 32 new per z-round
 constexpr int kSlots = 64;      // pending-exposure records (supersampled path): <= 31 + 32 alive
 constexpr int kPvRing = 4;      // parameter-vector records a warp keeps alive (single-passband path)
@@ -213,9 +216,12 @@ __device__ __forceinline__ void finish_exposure(const FluxArgs& A, const WarpSta
 
 // Table loads carry an L2 evict_last policy: the (k,z) table (60-160 MB) is re-read by every parameter vector while
 // gigabytes of write-once flux stream through the same L2 (those go out with evict-first stores).
+#ifndef PT_TABLE_POLICY
+#define PT_TABLE_POLICY "createpolicy.fractional.L2::evict_last.b64 %0, 1.0;"
+#endif
 __device__ __forceinline__ unsigned long long l2_keep_policy() {
   unsigned long long pol;
-  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+  asm volatile(PT_TABLE_POLICY : "=l"(pol));
   return pol;
 }
 __device__ __forceinline__ float ldg_keep(const float* p, unsigned long long pol) {
