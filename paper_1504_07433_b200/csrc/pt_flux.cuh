@@ -784,27 +784,27 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
           }
         }
       }
-      // append the in-window exposures to the exposure ring.  A lane rarely holds more than two of them (its exposures
-      // are 32*V apart), so the exclusive prefix of the per-lane counts is built from one ballot per count level.
-      if (__reduce_or_sync(0xffffffffu, inw)) {
+      // append the in-window exposures to the exposure ring, one 32-lane row (u) at a time: a transit is a run of
+      // consecutive exposures, so only one or two rows have any; per row two ballots give every lane its place, in
+      // time order, without divergence
+      unsigned rows = __reduce_or_sync(0xffffffffu, inw);
+      if (rows) {
         const unsigned lt = (1u << lane) - 1u;
-        const int cnt = __popc(inw);
-        int excl = 0, total = 0;
-        for (int level = 1;; ++level) {
-          const unsigned m = __ballot_sync(0xffffffffu, cnt >= level);
-          if (m == 0) break;
-          excl += __popc(m & lt);
-          total += __popc(m);
-        }
-        int pos = C.qhead + C.qcount + excl;
-        while (inw) {
-          const int b = __ffs(inw) - 1;
-          inw &= inw - 1u;
-          ws.expq[pos & (kExpQ - 1)] = (uint16_t)(base + ((b / V) * 32 + lane) * V + (b % V));
-          ++pos;
-        }
+        int tail = C.qhead + C.qcount;
+        do {
+          const int u = (__ffs(rows) - 1) / V;
+          rows &= ~(((1u << V) - 1u) << (u * V));
+          const unsigned pair = (inw >> (u * V)) & ((1u << V) - 1u);
+          const unsigned b0 = __ballot_sync(0xffffffffu, pair & 1u);
+          const unsigned b1 = (V == 2) ? __ballot_sync(0xffffffffu, pair & 2u) : 0u;
+          const int off = tail + __popc(b0 & lt) + __popc(b1 & lt);
+          const uint32_t e0 = base + (u * 32 + lane) * V;
+          if (pair & 1u) ws.expq[off & (kExpQ - 1)] = (uint16_t)e0;
+          if (V == 2 && (pair & 2u)) ws.expq[(off + (int)(pair & 1u)) & (kExpQ - 1)] = (uint16_t)(e0 + 1);
+          tail += __popc(b0) + __popc(b1);
+        } while (rows);
         __syncwarp();
-        C.qcount += total;
+        C.qcount = tail - C.qhead;
       }
       base += kSuper;
       } while (base < n_e && C.qcount < EPW);
