@@ -433,3 +433,51 @@ def test_per_passband_k_mode(pt, oracle, n_pv, n_pb, n_t, n_ss):
     assert np.abs(f - r).max() <= TOL64
     f32 = pt.pt_ma_quad_exact_pbk(dev(w.times), dev(w.params), n_pb, n_ss, w.t_exp, dtype=torch.float32).cpu().numpy()
     assert np.abs(f32 - r).max() <= TOL32
+
+
+# ------------------------------------------------------------------------------------------- window-test robustness
+def test_large_epochs_unsorted_times_and_padded_rows(pt, oracle):
+    """The cheap window test folds with t*(1/P) + c0; its error bound must hold for BJD-sized epochs (|t0/P| ~ 2e6),
+    negative times, unsorted and repeated times, NaN/inf times (flux 1), and rows padded beyond n_t."""
+    rng = np.random.default_rng(21)
+    n_pv, n_t = 12, 5000
+    P = rng.uniform(0.7, 9.0, n_pv)
+    a = rng.uniform(4, 15, n_pv)
+    b = rng.uniform(0, 0.9, n_pv)
+    e = np.where(np.arange(n_pv) % 2 == 0, 0.0, rng.uniform(0.05, 0.5, n_pv))
+    wv = rng.uniform(0, 2 * np.pi, n_pv)
+    inc = np.arccos(np.clip(b * (1 + e * np.sin(wv)) / (a * (1 - e * e)), -1, 1))
+    t0 = 2455000.0 + P * rng.uniform(0, 1, n_pv)
+    params = np.stack([t0, P, a, inc, e, wv, rng.uniform(0.03, 0.25, n_pv), 0.4 + 0 * P, 0.25 + 0 * P], 1)
+    times = 2455000.0 + rng.uniform(-400.0, 400.0, n_t)          # unsorted, ~800 d around the epochs
+    times[::97] = times[1::97][: len(times[::97])]                # repeated values
+    times[5], times[6], times[7] = np.nan, np.inf, -np.inf
+    for n_ss, t_exp in ((1, 0.0), (6, 0.02)):
+        w = inputs.Workload("bjd", times, params, 1, n_ss, t_exp)
+        f, r = gpu_exact(pt, w), ora_exact(oracle, w)
+        assert np.abs(f - r).max() <= TOL64
+        assert np.array_equal(f == 1.0, r == 1.0)
+    # the same through negative epochs and per-pv time rows with a padded stride
+    tt = np.full((n_pv, n_t + 37), 123.0)
+    for i in range(n_pv):
+        tt[i, :n_t] = -3.0e5 + np.sort(rng.uniform(-50, 50, n_t))
+    params[:, 0] = -3.0e5 + P * rng.uniform(0, 1, n_pv)
+    dt, dp = dev(tt), dev(params)
+    out = torch.empty((n_pv, 1, n_t), dtype=torch.float64, device="cuda")
+    from paper_1504_07433_b200 import binding
+    rc = binding.lib().pt_ma_quad_exact(dt.data_ptr(), n_t, n_t + 37, dp.data_ptr(), n_pv, 1, 3, 0.01, 0, out.data_ptr(), None,
+                                        torch.cuda.current_stream().cuda_stream)
+    assert rc == 0
+    torch.cuda.synchronize()
+    ref = oracle.ma_quad_exact(np.ascontiguousarray(tt[:, :n_t]), params, 1, 3, 0.01, prec="f128")
+    assert np.abs(out.cpu().numpy() - ref).max() <= TOL64
+
+
+def test_max_passbands_and_many_subsamples(pt, oracle):
+    """n_pb at the library's limit (1024: combine coefficients beyond the per-warp cache come from the row) and a
+    four-digit supersample count."""
+    w = inputs.config3(n_pv=3, n_pb=1024, n_t=64)
+    assert np.abs(gpu_exact(pt, w) - ora_exact(oracle, w)).max() <= TOL64
+    w = inputs.config2(n_pv=2, n_t=300)
+    w.n_ss, w.t_exp = 1500, 0.05
+    assert np.abs(gpu_exact(pt, w) - ora_exact(oracle, w)).max() <= TOL64
