@@ -11,7 +11,11 @@
 
 #include "pt_math.cuh"
 
+#ifndef PT_CEL_UNROLL
+#define PT_CEL_UNROLL 1
+#endif
 namespace pt {
+constexpr int kCelUnroll = PT_CEL_UNROLL;   // unroll factor of the AGM ladder loop
 
 struct Basis {
   double le, ld, ed;
@@ -28,7 +32,7 @@ __device__ __forceinline__ double cel_pair(double mc, double sp, double cK, doub
   // sequence 2: p2 = sqrt(1-n); b2 arrives already divided by p2
   double p2 = sp;
   double e = qc, em = 1.0;
-#pragma unroll 1
+#pragma unroll kCelUnroll
   for (int it = 0; it < 16; ++it) {
     const double rr = rcp_fast(em * p2);   // one reciprocal serves both sequences
     const double rem = rr * p2;
