@@ -281,6 +281,29 @@ def run_ours(args):
         res_i["workload"] = "BASELINE.json configs[3]: 4096 pv x 100000 times, table 401 x 12501, fp64 flux (3.28 GB/launch > L2)"
         extra["interp"] = res_i
         del it_, ip_, io
+    if rank == 0 and "configs" in sections:
+        # -------------------------------------------------------------- the other BASELINE configs, as specified
+        res_o = {}
+        w1 = inputs.config1()
+        a1, b1 = to_dev(w1.times), to_dev(w1.params)
+        o1 = torch.empty((1, 1, w1.n_t), dtype=torch.float64, device=dev)
+        t1 = _time_steps(lambda: pt.pt_ma_quad_exact(a1, b1, out=o1), 20, 3, None, 1) / 20
+        res_o["config1"] = {"latency_us": t1 * 1e6, "note": "1000 evaluations: a latency, not a throughput (SURVEY §8(d))"}
+        w3 = inputs.config3()
+        a3, b3 = to_dev(w3.times), to_dev(w3.params)
+        o3 = torch.empty((w3.n_pv, w3.n_pb, w3.n_t), dtype=torch.float64, device=dev)
+        t3 = _time_steps(lambda: pt.pt_ma_quad_exact(a3, b3, w3.n_pb, out=o3), 10, 3, flush, 1) / 10
+        t3k = _time_steps(lambda: pt.pt_ma_quad_exact_pbk(a3, b3, w3.n_pb, out=o3), 10, 3, flush, 1) / 10
+        res_o["config3"] = {"ms": t3 * 1e3, "z_evals_per_s": w3.n_pv * w3.n_t / t3, "fluxes_per_s": w3.n_pv * w3.n_pb * w3.n_t / t3,
+                            "exact_per_passband_k_ms": t3k * 1e3}
+        from oracle import pt_oracle as _po     # config 5's boundary-targeted times are solved on the oracle's orbit (inputs.py)
+        w5 = inputs.config5(lambda t, p: _po.orbit_z(t, p, prec="f64")[:, :, 0])
+        a5, b5 = to_dev(w5.times), to_dev(w5.params)
+        o5 = torch.empty((w5.n_pv, 1, w5.n_t), dtype=torch.float64, device=dev)
+        t5 = _time_steps(lambda: pt.pt_ma_quad_exact(a5, b5, out=o5), 10, 3, flush, 1) / 10
+        res_o["config5"] = {"ms": t5 * 1e3, "value": w5.n_eval / t5, "unit": UNIT}
+        extra["configs"] = res_o
+        del a1, b1, o1, a3, b3, o3, a5, b5, o5
     if rank == 0 and "chi2" in sections:
         # -------------------------------------------------------------- fused likelihood (S§8(f) NEXT-1): no flux is written
         res_c = {}
@@ -371,8 +394,8 @@ def main():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--sections", default="scaled,dense,interp,chi2,cpu",
-                    help="extra sections to run besides the headline: any of scaled,dense,interp,chi2,cpu (or 'none')")
+    ap.add_argument("--sections", default="scaled,dense,interp,configs,chi2,cpu",
+                    help="extra sections to run besides the headline: any of scaled,dense,interp,configs,chi2,cpu (or 'none')")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
