@@ -296,8 +296,8 @@ def run_ours(args):
         t3k = _time_steps(lambda: pt.pt_ma_quad_exact_pbk(a3, b3, w3.n_pb, out=o3), 10, 3, flush, 1) / 10
         res_o["config3"] = {"ms": t3 * 1e3, "z_evals_per_s": w3.n_pv * w3.n_t / t3, "fluxes_per_s": w3.n_pv * w3.n_pb * w3.n_t / t3,
                             "exact_per_passband_k_ms": t3k * 1e3}
-        from oracle import pt_oracle as _po     # config 5's boundary-targeted times are solved on the oracle's orbit (inputs.py)
-        w5 = inputs.config5(lambda t, p: _po.orbit_z(t, p, prec="f64")[:, :, 0])
+        # config 5's boundary-targeted times are solved on an orbit routine handed to the generator: here the product's own
+        w5 = inputs.config5(lambda t, p: pt.pt_orbit_z(to_dev(t), to_dev(p)).cpu().numpy()[:, :, 0])
         a5, b5 = to_dev(w5.times), to_dev(w5.params)
         o5 = torch.empty((w5.n_pv, 1, w5.n_t), dtype=torch.float64, device=dev)
         t5 = _time_steps(lambda: pt.pt_ma_quad_exact(a5, b5, out=o5), 10, 3, flush, 1) / 10
