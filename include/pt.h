@@ -80,9 +80,10 @@ int pt_ma_quad_exact(const double* d_times, int64_t n_t, int64_t t_stride_pv, co
 
 /* Exact per-passband-k mode (P:L177-L179 describe the mean-k evaluation above as an approximation):
  * every passband is evaluated with its OWN radius ratio k_j, i.e. flux[pv][j][:] equals pt_ma_quad_exact called with
- * n_pb = 1 on the row [t0,P,a,i,e,w,k_j,u1_j,u2_j].  Same arguments and layout as pt_ma_quad_exact; one launch per
- * passband on `stream` (the single-passband kernel reads passband j of the wide rows in place).  d_status[1] counts
- * affected (row, passband) pairs in this mode. */
+ * n_pb = 1 on the row [t0,P,a,i,e,w,k_j,u1_j,u2_j].  Same arguments and layout as pt_ma_quad_exact.  n_ss == 1: one fused
+ * launch (the orbit once per sample, the basis functions once per passband).  n_ss > 1: one launch per passband on
+ * `stream` (the single-passband kernel reads passband j of the wide rows in place; d_status[1] then counts affected
+ * (row, passband) pairs). */
 int pt_ma_quad_exact_pbk(const double* d_times, int64_t n_t, int64_t t_stride_pv, const double* d_params, int64_t n_pv,
                          int32_t n_pb, int32_t n_ss, double t_exp, int32_t dtype, void* d_flux, int32_t* d_status,
                          void* stream);

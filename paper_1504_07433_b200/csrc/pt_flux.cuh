@@ -67,6 +67,7 @@ struct FluxArgs {
   int pb_first;                // first passband of the row this launch looks at
   int64_t flux_pv_stride;      // flux elements between parameter vectors
   int64_t flux_off;            // flux element offset of this launch's first passband
+  int pbk;                     // 1: every passband at its own radius ratio, basis functions per passband (n_ss == 1 kernels)
   // fused likelihood (OutT = Chi2): observed flux and 1/sigma [n_pb][n_t] shared by all parameter vectors, chi2 [n_pv]
   const double* obs;
   const double* isig;
@@ -121,6 +122,7 @@ struct WarpState {
   PvRec pv[kPvRing];
   uint16_t expq[kExpQ];
   double coefc[3 * kCoefCache];
+  double kpb[kCoefCache];       // per-passband radius ratios (exact per-passband-k mode)
 };
 
 // The supersampled path's part of a warp's shared state (the n_ss == 1 kernels do not allocate it).
@@ -325,10 +327,11 @@ __device__ __noinline__ void tile_setup(const FluxArgs& A, WarpState& ws, int ri
     const double k = __ldg(pbp + 3 * j), u1 = __ldg(pbp + 3 * j + 1), u2 = __ldg(pbp + 3 * j + 2);
     const double N = 1.0 - u1 / 3.0 - u2 / 6.0;
     if (!(isfinite(k) && isfinite(u1) && isfinite(u2)) || !(k >= 0.0) || N == 0.0) ok = false;
-    ksum += k;
+    ksum = (!NPB1 && A.pbk) ? fmax(ksum, k) : ksum + k;
     if (j == 0) N0 = N;
   }
-  const double khat = NPB1 ? ksum : ksum / (double)n_pb;
+  // k̂: the mean radius ratio; per-passband-k mode: the largest one (window and in-transit test must cover all)
+  const double khat = (NPB1 || A.pbk) ? ksum : ksum / (double)n_pb;
   PvConst& c = r.c;          // all lanes store the same values
   c.khat = khat;
   pv_setup_orbit(c, row, ok, A.n_ss, A.t_exp);
@@ -369,10 +372,11 @@ __device__ __noinline__ void tile_setup(const FluxArgs& A, WarpState& ws, int ri
     for (int j = lane; j < n_pb && j < kCoefCache; j += 32) {
       const double k = __ldg(pbp + 3 * j), u1 = __ldg(pbp + 3 * j + 1), u2 = __ldg(pbp + 3 * j + 2);
       const double cj = u1 + 2.0 * u2;
-      const double gN = k * k * ik2 / (1.0 - u1 / 3.0 - u2 / 6.0);
+      const double gN = (A.pbk ? 1.0 : k * k * ik2) / (1.0 - u1 / 3.0 - u2 / 6.0);
       ws.coefc[3 * j + 0] = gN * (1.0 - cj);
       ws.coefc[3 * j + 1] = gN * cj;
       ws.coefc[3 * j + 2] = gN * u2;
+      ws.kpb[j] = k;
     }
   }
   if (MODE == 1) {
@@ -520,9 +524,28 @@ __device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, SsStat
     if (act) {
       const double zs = orbit_z_signed(r.c, fold_phase(t, r.c.t0, r.c.P, r.c.invP, slow_div));
       if (zs >= 0.0 && zs < 1.0 + khat) {
-        const Basis b = eval_basis<MODE>(A, r, zs);
-        if (NPB1) finish_exposure<true, OutT>(A, ws, r, e, fma(r.coef[2], b.ed, fma(r.coef[1], b.ld, r.coef[0] * b.le)), 0.0, 0.0, &chi_acc);
-        else finish_exposure<false, OutT>(A, ws, r, e, b.le, b.ld, b.ed, &chi_acc);
+        if (!NPB1 && MODE == 0 && A.pbk) {
+          // exact per-passband-k mode (S§8(f) NEXT-2): one orbit evaluation, the basis functions once per passband at k_j
+          double chi = 0.0;
+          for (int j = 0; j < n_pb; ++j) {
+            double kj, c0, c1, c2;
+            if (j < kCoefCache) {
+              kj = ws.kpb[j]; c0 = ws.coefc[3 * j]; c1 = ws.coefc[3 * j + 1]; c2 = ws.coefc[3 * j + 2];
+            } else {
+              const double u1 = __ldg(r.row + 7 + 3 * j), u2 = __ldg(r.row + 8 + 3 * j);
+              const double cj = u1 + 2.0 * u2, gN = 1.0 / (1.0 - u1 / 3.0 - u2 / 6.0);
+              kj = __ldg(r.row + 6 + 3 * j); c0 = gN * (1.0 - cj); c1 = gN * cj; c2 = gN * u2;
+            }
+            Basis b;
+            b.le = 0.0; b.ld = 0.0; b.ed = 0.0;
+            if (kj > 1.0e-150) b = ma_basis(kj, zs);
+            emit<OutT>(A, r, (OutT*)r.ob + e, e, j, fma(c2, b.ed, fma(c1, b.ld, c0 * b.le)), chi);
+          }
+        } else {
+          const Basis b = eval_basis<MODE>(A, r, zs);
+          if (NPB1) finish_exposure<true, OutT>(A, ws, r, e, fma(r.coef[2], b.ed, fma(r.coef[1], b.ld, r.coef[0] * b.le)), 0.0, 0.0, &chi_acc);
+          else finish_exposure<false, OutT>(A, ws, r, e, b.le, b.ld, b.ed, &chi_acc);
+        }
       } else {
         store_one<NPB1, OutT>(ob + e, A.n_t, n_pb);
       }

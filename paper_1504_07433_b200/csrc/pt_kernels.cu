@@ -168,6 +168,7 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   A.times = d_times; A.n_t = n_t; A.t_stride_pv = t_stride_pv; A.params = d_params; A.n_pv = n_pv;
   A.n_pb = n_pb; A.n_ss = n_ss; A.t_exp = t_exp; A.flux = d_flux; A.status = d_status;
   A.row_stride = 6 + 3 * (int64_t)n_pb; A.pb_first = 0; A.flux_pv_stride = (int64_t)n_pb * n_t; A.flux_off = 0;
+  A.pbk = (pb_view == -2) ? 1 : 0;
   if (pb_view >= 0) {   // single-passband view of passband `pb_view` in rows of n_pb_row passbands
     A.row_stride = 6 + 3 * (int64_t)n_pb_row; A.pb_first = pb_view;
     A.flux_pv_stride = (int64_t)n_pb_row * n_t; A.flux_off = (int64_t)pb_view * n_t;
@@ -294,6 +295,9 @@ int pt_ma_quad_exact_pbk(const double* d_times, int64_t n_t, int64_t t_stride_pv
                          void* stream) {
   int rc = check_common(d_times, d_params, d_flux, n_t, t_stride_pv, n_pv, n_pb, n_ss);
   if (rc) return rc;
+  if (n_ss == 1 && n_pb > 1)   // fused: one launch, the orbit once per sample, the basis functions once per passband
+    return launch_flux(0, nullptr, d_times, n_t, t_stride_pv, d_params, n_pv, n_pb, n_ss, t_exp, dtype, d_flux, d_status,
+                       (cudaStream_t)stream, nullptr, -2, n_pb);
   for (int j = 0; j < n_pb && rc == PT_OK; ++j)
     rc = launch_flux(0, nullptr, d_times, n_t, t_stride_pv, d_params, n_pv, 1, n_ss, t_exp, dtype, d_flux, d_status,
                      (cudaStream_t)stream, nullptr, j, n_pb);

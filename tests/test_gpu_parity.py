@@ -423,7 +423,7 @@ def test_chi2_interp_and_bad_rows(pt, oracle):
 
 
 # ------------------------------------------------------------------------------------------- exact per-passband k (NEXT-2)
-@pytest.mark.parametrize("n_pv,n_pb,n_t,n_ss", [(64, 20, 600, 1), (9, 3, 2501, 4), (200, 2, 33, 1)])
+@pytest.mark.parametrize("n_pv,n_pb,n_t,n_ss", [(64, 20, 600, 1), (9, 3, 2501, 4), (200, 2, 33, 1), (5, 40, 700, 1)])
 def test_per_passband_k_mode(pt, oracle, n_pv, n_pb, n_t, n_ss):
     w = inputs.config3(n_pv=n_pv, n_pb=n_pb, n_t=n_t)
     w.params[:, 6::3] *= np.linspace(0.7, 1.4, n_pb)[None, :]       # a wide spread of radius ratios
