@@ -328,12 +328,14 @@ def run_ours(args):
         from oracle import pt_oracle
         pt_oracle.build()
         n_cpu_pv = 64
-        t0 = time.perf_counter()
-        pt_oracle.ma_quad_exact(w.times, w.params[:n_cpu_pv], w.n_pb, w.n_ss, w.t_exp, prec="f64")
-        dt_cpu = time.perf_counter() - t0
+        dt_cpu = float("inf")
+        for _ in range(5):                                   # best of 5 wall-clock runs
+            t0 = time.perf_counter()
+            pt_oracle.ma_quad_exact(w.times, w.params[:n_cpu_pv], w.n_pb, w.n_ss, w.t_exp, prec="f64")
+            dt_cpu = min(dt_cpu, time.perf_counter() - t0)
         extra["cpu_baseline"] = {"value": n_cpu_pv * w.n_t * w.n_ss / dt_cpu, "unit": UNIT, "cores": pt_oracle.num_threads(),
                                  "kind": "oracle", "seconds": dt_cpu,
-                                 "sample": "all 64 pv of the same configs[1] batch, oracle double instantiation (OpenMP)"}
+                                 "sample": "all 64 pv of the same configs[1] batch (3.84e7 evals), oracle double instantiation (OpenMP), best of 5"}
 
     if rank == 0:
         line = {
