@@ -49,6 +49,13 @@ constexpr int kPvRing = 4;      // parameter-vector records a warp keeps alive (
 constexpr int kCoefCache = 32;  // passbands whose combine coefficients are cached per warp (multi-passband path)
 constexpr int kMaxTileLen = 32768;
 constexpr int kRemBias = 1 << 24;
+// -DPT_DEBUG_CHECKS: capacity invariants of the per-warp queues are checked and a violation traps (the test suite is run
+// once against such a build; compute-sanitizer is not available on the GPU pool).
+#ifdef PT_DEBUG_CHECKS
+#define PT_CHECK(cond) do { if (!(cond)) __trap(); } while (0)
+#else
+#define PT_CHECK(cond) do { } while (0)
+#endif
 #ifndef PT_EXPAND_INLINE
 #define PT_EXPAND_INLINE __forceinline__
 #endif
@@ -476,7 +483,11 @@ __device__ PT_BASIS_INLINE void basis_round(const FluxArgs& A, WarpState& ws, Ss
                                        (double)(s.acc[NACC - 2] + v[NACC - 2]) * A.fx_inv,
                                        (double)(s.acc[NACC - 1] + v[NACC - 1]) * A.fx_inv);
         }
+#ifdef PT_DEBUG_CHECKS
+        s.remaining = 0;
+#endif
       } else {
+        PT_CHECK(rem > 0);
         s.remaining = rem;
 #pragma unroll
         for (int a = 0; a < NACC; ++a) s.acc[a] += v[a];
@@ -579,6 +590,7 @@ __device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, SsStat
         if (act && g == 0) {
           if (has) {
             Slot& sl = ss.slots[sid];
+            PT_CHECK(sl.remaining == 0);
             sl.acc[0] = 0; sl.acc[1] = 0; sl.acc[2] = 0;
             sl.remaining = cnt; sl.e = (uint16_t)e; sl.ring = (uint16_t)cur;
           } else {
@@ -591,6 +603,7 @@ __device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, SsStat
           nalloc = 1;
           if (lane == 0) {
             Slot& sl = ss.slots[sid];
+            PT_CHECK(sl.remaining == 0);
             sl.acc[0] = 0; sl.acc[1] = 0; sl.acc[2] = 0;
             sl.remaining = kRemBias; sl.e = (uint16_t)e; sl.ring = (uint16_t)cur;
           }
@@ -605,6 +618,7 @@ __device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, SsStat
       }
       __syncwarp();
       C.icount += __popc(m);
+      PT_CHECK(C.icount <= kItemQ);
       C.slot_next = (C.slot_next + nalloc) & (kSlots - 1);
     }
     if (multi) {
@@ -672,6 +686,10 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
   SsState& ss = s_ss[SS1 ? 0 : (threadIdx.x >> 5)];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   WarpState& ws = s_ws[warp];
+#ifdef PT_DEBUG_CHECKS
+  if (!SS1) for (int i = lane; i < kSlots; i += 32) ss.slots[i].remaining = 0;
+  __syncwarp();
+#endif
   WarpCtr C;
   C.qhead = 0; C.qcount = 0; C.ihead = 0; C.icount = 0; C.slot_next = 0; C.cur = 0;
   const int n_pb = NPB1 ? 1 : A.n_pb;
@@ -828,6 +846,7 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
         } while (rows);
         __syncwarp();
         C.qcount = tail - C.qhead;
+        PT_CHECK(C.qcount <= kExpQ);
       }
       base += kSuper;
       } while (base < n_e && C.qcount < EPW);
