@@ -49,6 +49,7 @@ constexpr int kPvRing = 4;      // parameter-vector records a warp keeps alive (
 constexpr int kCoefCache = 32;  // passbands whose combine coefficients are cached per warp (multi-passband path)
 constexpr int kMaxTileLen = 32768;
 constexpr int kRemBias = 1 << 24;
+constexpr int kLptMax = 512;    // parameter vectors that the longest-processing-time-first order is built for
 // -DPT_DEBUG_CHECKS: capacity invariants of the per-warp queues are checked and a violation traps (the test suite is run
 // once against such a build; compute-sanitizer is not available on the GPU pool).
 #ifdef PT_DEBUG_CHECKS
@@ -87,6 +88,7 @@ struct FluxArgs {
   int64_t n_tiles;
   unsigned long long* sched;   // scheduler slot: [0] global tile ticket, [1] warps that have finished, [2+pv] per-pv tickets
   int per_pv;                  // 1: warps stay on one parameter vector and take its tiles from sched[2+pv] (n_pv small)
+  int lpt;                     // 1: global mode with the parameter vectors in order of decreasing expected work (n_pv <= kLptMax)
   // supersample accumulation (fixed point)
   int fx_bits;             // 61 - ceil(log2 n_ss): a sum of n_ss values below 2^eb fits an int64 at scale 2^(fx_bits-eb)
   double fx_scale;         // 2^fx_bits (basis values are <= 1)
@@ -712,6 +714,33 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
   //     parameter vector (setup done once, later tiles only move the tile pointers) and moves on to the next one that has
   //     tiles left when it is exhausted, so fast parameter vectors lend their warps to slow ones.
   // The last warp to finish zeroes the slot for the next launch that uses it.
+  // LPT order: tiles of rows with many (long) transits are dealt first, so that the launch ends on light tiles.  The
+  // expected work of a row is its in-window fraction, roughly sqrt((1+k)² - b²) / (π a) + t_exp / P; the estimate only
+  // orders the tiles.  One block barrier, before any warp starts its pipeline.
+  __shared__ uint16_t s_weight[kLptMax];   // quantised: it only has to order the rows
+  __shared__ uint16_t s_order[kLptMax];
+  if (A.lpt) {
+    const int n = (int)A.n_pv;
+    for (int i = threadIdx.x; i < n; i += kThreads) {
+      const double* row = A.params + (int64_t)i * A.row_stride;
+      const double P = row[1], a = row[2], ci = cos(row[3]), k = row[6 + 3 * A.pb_first];
+      const double b = a * ci, c2 = (1.0 + k) * (1.0 + k) - b * b;
+      float wgt = (float)(sqrt(fmax(c2, 0.0)) / (3.14159 * a) + ((A.n_ss > 1) ? fabs(A.t_exp / P) : 0.0));
+      if (!(wgt == wgt) || wgt > 1.0f) wgt = 1.0f;    // odd rows (eccentric, bad parameters): treat as heavy
+      s_weight[i] = (uint16_t)(wgt * 65535.0f);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < n; i += kThreads) {
+      const unsigned wi = s_weight[i];
+      int rank = 0;
+      for (int j = 0; j < n; ++j) {
+        const unsigned wj = s_weight[j];
+        rank += (wj > wi || (wj == wi && j < i)) ? 1 : 0;
+      }
+      s_order[rank] = (uint16_t)i;
+    }
+    __syncthreads();
+  }
   const int tpp = A.tiles_per_pv;
   int64_t pv_cur = 0, last_pv = -1;
   int chunk_cur = 0, last_ring = -1;
@@ -720,6 +749,7 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
     have = gw < A.n_tiles;
     pv_cur = gw / tpp;
     chunk_cur = (int)(gw - pv_cur * tpp);
+    if (A.lpt && have) pv_cur = s_order[pv_cur];
   } else {
     pv_cur = gw % A.n_pv;
     unsigned long long f0 = 0;
@@ -778,6 +808,7 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
           have = tile < A.n_tiles;
           pv_cur = tile / tpp;
           chunk_cur = (int)(tile - pv_cur * tpp);
+          if (A.lpt && have) pv_cur = s_order[pv_cur];
         } else if (nf < (unsigned long long)tpp) {
           chunk_cur = (int)nf;
         } else {

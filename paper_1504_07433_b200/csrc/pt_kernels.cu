@@ -189,10 +189,18 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   tl = (tl + 255) / 256 * 256;
   if (tl < 256) tl = 256;
   if (tl > 16384) tl = 16384;
-  const int64_t tpp = (n_t + tl - 1) / tl;
+  int64_t tpp = (n_t + tl - 1) / tl;
   if (tpp > 0x7fffffff || (double)tpp * (double)n_pv > 9.0e18) return PT_ERR_SIZE;
   A.tile_len = (int)tl; A.tiles_per_pv = (int)tpp; A.n_tiles = n_pv * tpp;
   A.per_pv = (n_pv <= kSchedWords - 2 - kBaseBlocks && tpp >= 2) ? 1 : 0;   // the slot's tail holds the chi2 partials
+#ifndef PT_LPT_TILE
+#define PT_LPT_TILE 512
+#endif
+  A.lpt = (A.per_pv && n_pv <= kLptMax) ? 1 : 0;
+  if (A.lpt) {
+    A.per_pv = 0;
+    if (tl < PT_LPT_TILE) { tl = PT_LPT_TILE; tpp = (n_t + tl - 1) / tl; }
+  }
   int lg = 0;
   while (((int64_t)1 << lg) < (int64_t)n_ss) ++lg;
   A.fx_bits = 61 - lg;
