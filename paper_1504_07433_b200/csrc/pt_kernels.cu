@@ -196,7 +196,7 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
 #ifndef PT_LPT_TILE
 #define PT_LPT_TILE 512
 #endif
-  A.lpt = (A.per_pv && n_pv <= kLptMax) ? 1 : 0;
+  A.lpt = (A.per_pv && n_pv <= kLptMax && n_pv * tpp >= 2 * warps) ? 1 : 0;   // worth ranking the rows only with several tiles per warp
   if (A.lpt) {
     A.per_pv = 0;
     if (tl < PT_LPT_TILE) { tl = PT_LPT_TILE; tpp = (n_t + tl - 1) / tl; }
