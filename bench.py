@@ -37,9 +37,9 @@ ALG_PER_TRANSIT_ECC = 900.0   # the same with the Newton–Kepler solve
 FP64_LANES_PER_SM, N_SM = 64, 148
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/r1c_ncu_*.md);
 # a kernel's output that is still in L2 when the capture ends is not in its figure (configs[1]: 30.7 MB of flux < 126 MB L2).
-TRAFFIC_EXACT_CONFIG2 = 558.336e3 + 6.656e3
-TRAFFIC_INTERP_F32 = 524.876800e6 + 3.234138e9
-TRAFFIC_DENSE = 134.706176e6 + 87.616256e6
+TRAFFIC_EXACT_CONFIG2 = 563.456e3 + 3.328e3
+TRAFFIC_INTERP_F32 = 519.879936e6 + 3.233794e9
+TRAFFIC_DENSE = 134.598656e6 + 88.509696e6
 
 
 def _peaks():
