@@ -717,29 +717,47 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
   // LPT order: tiles of rows with many (long) transits are dealt first, so that the launch ends on light tiles.  The
   // expected work of a row is its in-window fraction, roughly sqrt((1+k)² - b²) / (π a) + t_exp / P; the estimate only
   // orders the tiles.  One block barrier, before any warp starts its pipeline.
-  __shared__ uint16_t s_weight[kLptMax];   // quantised: it only has to order the rows
-  __shared__ uint16_t s_order[kLptMax];
+  __shared__ uint32_t s_key[kLptMax];      // (quantised weight << 16) | (0xffff - row): unique keys, sorted descending
   if (A.lpt) {
     const int n = (int)A.n_pv;
-    for (int i = threadIdx.x; i < n; i += kThreads) {
-      const double* row = A.params + (int64_t)i * A.row_stride;
-      const double P = row[1], a = row[2], ci = cos(row[3]), k = row[6 + 3 * A.pb_first];
-      const double b = a * ci, c2 = (1.0 + k) * (1.0 + k) - b * b;
-      float wgt = (float)(sqrt(fmax(c2, 0.0)) / (3.14159 * a) + ((A.n_ss > 1) ? fabs(A.t_exp / P) : 0.0));
-      if (!(wgt == wgt) || wgt > 1.0f) wgt = 1.0f;    // odd rows (eccentric, bad parameters): treat as heavy
-      s_weight[i] = (uint16_t)(wgt * 65535.0f);
-    }
-    __syncthreads();
-    for (int i = threadIdx.x; i < n; i += kThreads) {
-      const unsigned wi = s_weight[i];
-      int rank = 0;
-      for (int j = 0; j < n; ++j) {
-        const unsigned wj = s_weight[j];
-        rank += (wj > wi || (wj == wi && j < i)) ? 1 : 0;
+    int np2 = 32;
+    while (np2 < n) np2 <<= 1;
+    for (int i = threadIdx.x; i < np2; i += kThreads) {
+      uint32_t key = 0u;                                  // padding sorts last
+      if (i < n) {
+        const double* row = A.params + (int64_t)i * A.row_stride;
+        const double P = row[1], a = row[2], ci = cos(row[3]), k = row[6 + 3 * A.pb_first];
+        const double b = a * ci, c2 = (1.0 + k) * (1.0 + k) - b * b;
+        float wgt = (float)(sqrt(fmax(c2, 0.0)) / (3.14159 * a) + ((A.n_ss > 1) ? fabs(A.t_exp / P) : 0.0));
+        if (!(wgt == wgt) || wgt > 1.0f) wgt = 1.0f;      // odd rows (bad parameters, a < 1+k): treat as heavy
+        key = ((uint32_t)(wgt * 65535.0f) << 16) | (uint32_t)(0xffff - i);
       }
-      s_order[rank] = (uint16_t)i;
+      s_key[i] = key;
     }
     __syncthreads();
+    if (n <= 128) {                                       // few rows: rank by counting (one more barrier instead of ~28)
+      uint32_t mine = 0u;
+      int rank = 0;
+      if ((int)threadIdx.x < n) {
+        mine = s_key[threadIdx.x];
+        for (int j = 0; j < n; ++j) rank += (s_key[j] > mine) ? 1 : 0;
+      }
+      __syncthreads();
+      if ((int)threadIdx.x < n) s_key[rank] = mine;
+      __syncthreads();
+    } else
+    for (int size = 2; size <= np2; size <<= 1) {         // bitonic sort, descending
+      for (int stride = size >> 1; stride > 0; stride >>= 1) {
+        for (int t = threadIdx.x; t < (np2 >> 1); t += kThreads) {
+          const int lo = 2 * t - (t & (stride - 1));
+          const int hi = lo + stride;
+          const bool desc = (lo & size) == 0;
+          const uint32_t x = s_key[lo], y = s_key[hi];
+          if ((x < y) == desc) { s_key[lo] = y; s_key[hi] = x; }
+        }
+        __syncthreads();
+      }
+    }
   }
   const int tpp = A.tiles_per_pv;
   int64_t pv_cur = 0, last_pv = -1;
@@ -749,7 +767,7 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
     have = gw < A.n_tiles;
     pv_cur = gw / tpp;
     chunk_cur = (int)(gw - pv_cur * tpp);
-    if (A.lpt && have) pv_cur = s_order[pv_cur];
+    if (A.lpt && have) pv_cur = 0xffff - (int)(s_key[pv_cur] & 0xffffu);
   } else {
     pv_cur = gw % A.n_pv;
     unsigned long long f0 = 0;
@@ -808,7 +826,7 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
           have = tile < A.n_tiles;
           pv_cur = tile / tpp;
           chunk_cur = (int)(tile - pv_cur * tpp);
-          if (A.lpt && have) pv_cur = s_order[pv_cur];
+          if (A.lpt && have) pv_cur = 0xffff - (int)(s_key[pv_cur] & 0xffffu);
         } else if (nf < (unsigned long long)tpp) {
           chunk_cur = (int)nf;
         } else {
