@@ -1,14 +1,17 @@
 // pt_flux.cuh — the fused flux kernel: S0-S7 (and S9) of the hot path in one persistent launch.
 //
-// Every warp is an autonomous pipeline; the block is only a container (no block barrier anywhere).  A warp takes tiles
-// (parameter vector pv, run of `tile_len` exposures) in a strided order and pushes the work through three stages, each of
-// which runs with (nearly) all 32 lanes busy because the stages are decoupled by per-warp queues in shared memory:
+// Every warp is an autonomous pipeline; the block is only a container (no block barrier once the pipelines run).  A warp
+// takes tiles (parameter vector pv, run of `tile_len` exposures) from counters in the launch's scheduler slot — heaviest
+// rows first when the population is small enough to rank (LPT order), else in index order or per parameter vector — and
+// pushes the work through three stages, each of which runs with (nearly) all 32 lanes busy because the stages are
+// decoupled by per-warp queues in shared memory:
 //
 //   stream   every exposure of the tile: 16-byte time loads, a 6-instruction phase-window test, flux = 1 written with
 //            16-byte streaming stores for the exposures that cannot be in transit; the others go to the EXPOSURE queue
 //   z-stage  G = min(n_ss,32) lanes per queued exposure: pinned subsample time + phase fold (H1, H2), orbit -> signed z
 //            (Newton–Kepler for e > 0).  Subsamples with 0 <= z < 1+k̂ are compacted (ballot + popc, order kept) into
-//            the ITEM queue; an exposure without any such subsample is finished here (flux = 1)
+//            the ITEM queue; an exposure without any such subsample is finished here (flux = 1).  n_ss == 1: the basis
+//            functions are evaluated in this round (an in-window exposure is almost always in transit)
 //   basis    32 queued subsamples, possibly of different exposures, tiles and parameter vectors: λe, λd*, ηd by the closed
 //            forms / one shared `cel` ladder (pt_basis.cuh) or the bilinear table lookup; the supersample sum is a
 //            segmented warp-shuffle reduction over the lanes that belong to one exposure, in 64-bit fixed point so that
