@@ -60,6 +60,9 @@ constexpr int kLptMax = 512;    // parameter vectors that the longest-processing
 #else
 #define PT_CHECK(cond) do { } while (0)
 #endif
+#ifndef PT_ST
+#define PT_ST __stcs   // flux stores: write-once data, evict-first
+#endif
 #ifndef PT_EXPAND_INLINE
 #define PT_EXPAND_INLINE __forceinline__
 #endif
@@ -169,8 +172,8 @@ __device__ __forceinline__ void store_one(OutT* __restrict__ out, int64_t n_t, i
   if constexpr (kIsChi2<OutT>) {
     return;   // flux 1 is what the chi2 baseline assumes: nothing to add
   } else {
-    if (NPB1) __stcs(out, (OutT)1.0);
-    else for (int j = 0; j < n_pb; ++j) __stcs(out + (int64_t)j * n_t, (OutT)1.0);
+    if (NPB1) PT_ST(out, (OutT)1.0);
+    else for (int j = 0; j < n_pb; ++j) PT_ST(out + (int64_t)j * n_t, (OutT)1.0);
   }
 }
 template <bool NPB1, typename OutT>
@@ -180,8 +183,8 @@ __device__ __forceinline__ void store_one_pair(OutT* __restrict__ out, int64_t n
   } else {
     typename Vec2<OutT>::type v;
     v.x = (OutT)1.0; v.y = (OutT)1.0;
-    if (NPB1) __stcs((typename Vec2<OutT>::type*)out, v);
-    else for (int j = 0; j < n_pb; ++j) __stcs((typename Vec2<OutT>::type*)(out + (int64_t)j * n_t), v);
+    if (NPB1) PT_ST((typename Vec2<OutT>::type*)out, v);
+    else for (int j = 0; j < n_pb; ++j) PT_ST((typename Vec2<OutT>::type*)(out + (int64_t)j * n_t), v);
   }
 }
 
@@ -197,7 +200,7 @@ __device__ __forceinline__ void emit(const FluxArgs& A, const PvRec& r, OutT* ou
     const double o = __ldg(A.obs + idx), w = __ldg(A.isig + idx);
     chi = fma(dec * w * w, fma(2.0, o - 1.0, dec), chi);
   } else {
-    __stcs(out + (int64_t)j * A.n_t, (OutT)(1.0 - dec));
+    PT_ST(out + (int64_t)j * A.n_t, (OutT)(1.0 - dec));
   }
 }
 
