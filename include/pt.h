@@ -137,6 +137,12 @@ int pt_ma_quad_interp_host(const pt_table* table, const double* h_times, int64_t
  * d_sink[blocks*256] so the work cannot be removed.  FP64 thread-instructions issued = blocks*256*iters*8. */
 int pt_probe_dfma(int32_t blocks, int32_t iters, double* d_sink, void* stream);
 
+/* How the flux kernels would cut up a problem on a device with n_sm multiprocessors (pure host logic, no CUDA call; used
+ * by the CPU tests).  h_out[0] = exposures per tile, [1] = tiles per parameter vector, [2] = scheduling mode (0 global
+ * tile counter, 1 one counter per parameter vector, 2 global counter with rows in longest-processing-time-first order),
+ * [3] = blocks of 256 threads in the persistent grid. */
+int pt_plan(int64_t n_pv, int64_t n_t, int32_t n_sm, int64_t* h_out);
+
 /* Number of kernel launches the library has enqueued so far in this process (bench.py's gpu_launches evidence). */
 int64_t pt_launch_count(void);
 

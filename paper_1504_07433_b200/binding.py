@@ -21,7 +21,7 @@ PT_ST_BAD_PARAM, PT_ST_K_OUT_OF_TABLE = 1, 2
 _ERR = {1: "PT_ERR_NULL", 2: "PT_ERR_SIZE", 3: "PT_ERR_DTYPE", 4: "PT_ERR_TABLE", 5: "PT_ERR_CUDA"}
 
 EXPORTS = ("pt_build_arch", "pt_orbit_z", "pt_ma_quad_exact", "pt_ma_table_build", "pt_ma_quad_interp", "pt_ma_quad_chi2", "pt_ma_quad_exact_pbk",
-           "pt_ma_quad_exact_host", "pt_ma_quad_interp_host", "pt_probe_dfma", "pt_launch_count")
+           "pt_ma_quad_exact_host", "pt_ma_quad_interp_host", "pt_plan", "pt_probe_dfma", "pt_launch_count")
 
 
 class PtError(RuntimeError):
@@ -57,6 +57,7 @@ def lib() -> C.CDLL:
         L.pt_ma_quad_exact_host.argtypes = common + [i32, ptr, ptr]
         L.pt_ma_quad_interp_host.argtypes = [C.POINTER(pt_table)] + common + [i32, ptr, ptr]
         L.pt_probe_dfma.argtypes = [i32, i32, ptr, ptr]
+        L.pt_plan.argtypes = [i64, i64, i32, C.POINTER(C.c_int64)]
         for n in EXPORTS[1:-1]:
             getattr(L, n).restype = C.c_int
         _lib = L
@@ -217,6 +218,13 @@ def pt_probe_dfma(blocks: int, iters: int, sink: torch.Tensor) -> None:
     if not sink.is_cuda or sink.dtype != torch.float64 or sink.numel() < blocks * 256:
         raise PtError("sink must be a CUDA float64 tensor of at least blocks*256 elements")
     _check(lib().pt_probe_dfma(blocks, iters, sink.data_ptr(), _stream()), "pt_probe_dfma")
+
+
+def pt_plan(n_pv: int, n_t: int, n_sm: int = 148) -> dict:
+    """Tiling and scheduling mode the flux kernels would use (include/pt.h: pt_plan); host logic only, works without a GPU."""
+    out = (C.c_int64 * 4)()
+    _check(lib().pt_plan(n_pv, n_t, n_sm, out), "pt_plan")
+    return {"tile_len": int(out[0]), "tiles_per_pv": int(out[1]), "mode": int(out[2]), "blocks": int(out[3])}
 
 
 def pt_launch_count() -> int:

@@ -152,6 +152,46 @@ static int sm_count() {
   return n;
 }
 
+// How a launch is cut up (pure host logic; exported as pt_plan for the CPU tests).
+//   persistent grid: PT_MIN_BLOCKS blocks of 8 autonomous warps per SM; tiles of `tile_len` exposures of one parameter
+//   vector, about kTilesPerWarp per warp so that heavy and light tiles average out.
+//   mode 0  one global tile counter, rows in index order
+//   mode 1  one counter per parameter vector (a warp keeps its parameter vector: the setup is reused)
+//   mode 2  global counter, rows in order of decreasing expected work (LPT): heavy tiles first, the launch ends on light ones
+struct Plan {
+  int tile_len;
+  int64_t tiles_per_pv;
+  int mode;
+  int64_t blocks;
+};
+#ifndef PT_LPT_TILE
+#define PT_LPT_TILE 256
+#endif
+static Plan plan_tiles(int64_t n_pv, int64_t n_t, int n_sm) {
+  Plan p{};
+  const int64_t warps = (int64_t)n_sm * PT_MIN_BLOCKS * kWarpsPerBlock;
+  constexpr int64_t kTilesPerWarp = 8;
+  const double total = (double)n_pv * (double)n_t;
+  int64_t tl = (int64_t)(total / (double)(warps * kTilesPerWarp));
+  tl = (tl + 255) / 256 * 256;
+  if (tl < 256) tl = 256;
+  if (tl > 16384) tl = 16384;
+  int64_t tpp = (n_t + tl - 1) / tl;
+  const bool few = (n_pv <= kSchedWords - 2 - kBaseBlocks && tpp >= 2);   // the slot's tail holds the chi2 partials
+  p.mode = few ? 1 : 0;
+  if (few && n_pv <= kLptMax && n_pv * tpp >= 2 * warps) {   // worth ranking the rows only with several tiles per warp
+    p.mode = 2;
+    if (tl < PT_LPT_TILE) { tl = PT_LPT_TILE; tpp = (n_t + tl - 1) / tl; }
+  }
+  if (tpp > 0x7fffffff || (double)tpp * (double)n_pv > 9.0e18) return p;   // tile_len == 0: too large
+  p.tile_len = (int)tl;
+  p.tiles_per_pv = tpp;
+  const int64_t n_tiles = n_pv * tpp;
+  p.blocks = (n_tiles + kWarpsPerBlock - 1) / kWarpsPerBlock;
+  if (p.blocks > warps / kWarpsPerBlock) p.blocks = warps / kWarpsPerBlock;
+  return p;
+}
+
 struct Chi2Args {
   const double* obs;
   const double* isig;
@@ -180,36 +220,17 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
     A.tb = tb->d_data; A.tb_dtype = tb->dtype; A.n_k = tb->n_k; A.n_z = tb->n_z; A.n_fn = tb->n_fn;
     A.k_min = tb->k_min; A.dk = tb->dk; A.dz = tb->dz;
   }
-  // persistent grid: PT_MIN_BLOCKS blocks of 8 autonomous warps per SM; tiles of `tile_len` exposures of one parameter
-  // vector are dealt to the warps in strided order, about kTilesPerWarp each so that heavy and light tiles average out
-  const int64_t warps = (int64_t)sm_count() * PT_MIN_BLOCKS * kWarpsPerBlock;
-  constexpr int64_t kTilesPerWarp = 8;
-  const double total = (double)n_pv * (double)n_t;
-  int64_t tl = (int64_t)(total / (double)(warps * kTilesPerWarp));
-  tl = (tl + 255) / 256 * 256;
-  if (tl < 256) tl = 256;
-  if (tl > 16384) tl = 16384;
-  int64_t tpp = (n_t + tl - 1) / tl;
-  if (tpp > 0x7fffffff || (double)tpp * (double)n_pv > 9.0e18) return PT_ERR_SIZE;
-  A.tile_len = (int)tl; A.tiles_per_pv = (int)tpp; A.n_tiles = n_pv * tpp;
-  A.per_pv = (n_pv <= kSchedWords - 2 - kBaseBlocks && tpp >= 2) ? 1 : 0;   // the slot's tail holds the chi2 partials
-#ifndef PT_LPT_TILE
-#define PT_LPT_TILE 512
-#endif
-  A.lpt = (A.per_pv && n_pv <= kLptMax && n_pv * tpp >= 2 * warps) ? 1 : 0;   // worth ranking the rows only with several tiles per warp
-  if (A.lpt) {
-    A.per_pv = 0;
-    if (tl < PT_LPT_TILE) { tl = PT_LPT_TILE; tpp = (n_t + tl - 1) / tl; }
-  }
+  const pt::Plan plan = plan_tiles(n_pv, n_t, sm_count());
+  if (plan.tile_len == 0) return PT_ERR_SIZE;
+  A.tile_len = plan.tile_len; A.tiles_per_pv = (int)plan.tiles_per_pv; A.n_tiles = n_pv * plan.tiles_per_pv;
+  A.per_pv = plan.mode == 1; A.lpt = plan.mode == 2;
   int lg = 0;
   while (((int64_t)1 << lg) < (int64_t)n_ss) ++lg;
   A.fx_bits = 61 - lg;
   A.fx_scale = ldexp(1.0, A.fx_bits);
   A.fx_inv = 1.0 / (A.fx_scale * (double)n_ss);
   A.inv_nss = 1.0 / (double)n_ss;
-  int64_t blocks = (A.n_tiles + kWarpsPerBlock - 1) / kWarpsPerBlock;
-  if (blocks > warps / kWarpsPerBlock) blocks = warps / kWarpsPerBlock;
-  const dim3 grid((unsigned)blocks);
+  const dim3 grid((unsigned)plan.blocks);
   A.sched = sched_slot();
   if (!A.sched) return PT_ERR_CUDA;
   if (dtype == kDtypeChi2) {
@@ -267,6 +288,15 @@ int pt_build_arch(void) {
 }
 
 int64_t pt_launch_count(void) { return g_launches.load(); }
+
+int pt_plan(int64_t n_pv, int64_t n_t, int32_t n_sm, int64_t* h_out) {
+  if (!h_out) return PT_ERR_NULL;
+  if (n_pv <= 0 || n_t <= 0 || n_sm <= 0) return PT_ERR_SIZE;
+  const Plan p = plan_tiles(n_pv, n_t, n_sm);
+  if (p.tile_len == 0) return PT_ERR_SIZE;
+  h_out[0] = p.tile_len; h_out[1] = p.tiles_per_pv; h_out[2] = p.mode; h_out[3] = p.blocks;
+  return PT_OK;
+}
 
 int pt_probe_dfma(int32_t blocks, int32_t iters, double* d_sink, void* stream) {
   if (!d_sink) return PT_ERR_NULL;

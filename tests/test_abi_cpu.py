@@ -99,3 +99,34 @@ def test_input_generators_are_seeded_and_shaped():
     assert k.min() >= 0.05 and k.max() <= 0.2
     u1, u2 = a.params[:, 7], a.params[:, 8]
     assert np.all(u1 + u2 <= 1 + 1e-12) and np.all(u1 >= 0) and np.all(u1 + 2 * u2 >= -1e-12)   # Kipping's triangle
+
+
+def test_launch_plan_host_logic(libpath):
+    """Tiling / scheduling decisions of the host side (pt_plan: no CUDA call), for the five BASELINE shapes on 148 SMs."""
+    from paper_1504_07433_b200 import binding
+    warps = 148 * 3 * 8
+    # configs[1]: 64 rows of 60000 -> few rows, many tiles per warp: longest-processing-time-first order, full grid
+    p = binding.pt_plan(64, 60000)
+    assert p["mode"] == 2 and p["tile_len"] % 256 == 0 and p["blocks"] == 148 * 3
+    assert p["tiles_per_pv"] == -(-60000 // p["tile_len"]) and 64 * p["tiles_per_pv"] >= 2 * warps
+    # configs[0]: one short row -> one block is enough, a global counter
+    p = binding.pt_plan(1, 1000)
+    assert p["mode"] in (0, 1) and p["blocks"] == 1 and p["tile_len"] * p["tiles_per_pv"] >= 1000
+    # configs[2]: 512 rows of 600 -> fewer tiles than warps: no ranking, per-row counters
+    p = binding.pt_plan(512, 600)
+    assert p["mode"] == 1 and p["tiles_per_pv"] == 3
+    # configs[3]: 4096 rows of 100000 -> too many rows for per-row counters: global counter, long tiles, full grid
+    p = binding.pt_plan(4096, 100000)
+    assert p["mode"] == 0 and p["tile_len"] == 14592 and p["tiles_per_pv"] == 7 and p["blocks"] == 148 * 3
+    # configs[4]: 4096 rows of 4096
+    p = binding.pt_plan(4096, 4096)
+    assert p["mode"] == 0 and p["tile_len"] * p["tiles_per_pv"] >= 4096 and p["blocks"] == 148 * 3
+    # every exposure is covered exactly once whatever the shape; the grid never exceeds three blocks per SM
+    for n_pv, n_t, n_sm in ((1, 1, 148), (3, 255, 148), (3, 257, 132), (1000, 7, 148), (7, 10 ** 7, 148), (10 ** 6, 3, 148),
+                            (448, 60000, 148), (2, 2 ** 31 - 1, 8)):
+        p = binding.pt_plan(n_pv, n_t, n_sm)
+        assert 256 <= p["tile_len"] <= 16384 and p["tile_len"] % 256 == 0
+        assert (p["tiles_per_pv"] - 1) * p["tile_len"] < n_t <= p["tiles_per_pv"] * p["tile_len"]
+        assert 1 <= p["blocks"] <= n_sm * 3
+    with pytest.raises(binding.PtError):
+        binding.pt_plan(0, 10)
