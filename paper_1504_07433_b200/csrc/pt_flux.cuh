@@ -351,7 +351,7 @@ __device__ __noinline__ void tile_setup(const FluxArgs& A, WarpState& ws, int ri
   c.khat = khat;
   pv_setup_orbit(c, row, ok, A.n_ss, A.t_exp);
   const int64_t e0 = (int64_t)chunk * A.tile_len;
-  const double ik2 = khat > 1.0e-150 ? rcp_fast(khat * khat) : (khat > 0.0 ? 1.0 / (khat * khat) : 0.0);
+  const double ik2 = NPB1 ? 1.0 : (khat > 1.0e-150 ? rcp_fast(khat * khat) : (khat > 0.0 ? 1.0 / (khat * khat) : 0.0));   // single passband: unused
   if (lane == 0) {
     r.tb = A.times + pv * A.t_stride_pv + e0;
     r.ob = kIsChi2<OutT> ? nullptr : (char*)A.flux + (pv * A.flux_pv_stride + A.flux_off + e0) * (int64_t)sizeof(OutT);

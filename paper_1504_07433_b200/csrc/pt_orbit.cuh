@@ -163,8 +163,8 @@ __device__ __forceinline__ double asin_unit(double x) {
 // Validate a parameter row and fill the orbit part of PvConst (khat is set by the caller beforehand).
 // `row` = [t0, P, a/R*, i, e, w, ...]; half_exp_phase = half the exposure in cycles (0 when n_ss == 1).
 __device__ __forceinline__ void pv_setup_orbit(PvConst& c, const double* row, bool row_ok, int n_ss, double t_exp) {
-  const double t0 = row[0], P = row[1], a = row[2], inc = row[3], e = row[4];
-  double w = row[5];
+  const double t0 = __ldg(row), P = __ldg(row + 1), a = __ldg(row + 2), inc = __ldg(row + 3), e = __ldg(row + 4);
+  double w = __ldg(row + 5);
   int flags = 0;
   if (!row_ok || !(isfinite(t0) && isfinite(P) && isfinite(a) && isfinite(inc) && isfinite(e) && isfinite(w)) ||
       !(P > 0.0) || !(a > 0.0) || !(e >= 0.0 && e < 1.0)) {
