@@ -67,6 +67,8 @@ constexpr int kLptMax = 512;    // parameter vectors that the longest-processing
 #define PT_EXPAND_INLINE __forceinline__
 #endif
 
+struct PvRec;
+
 struct FluxArgs {
   const double* times;
   int64_t n_t, t_stride_pv;
@@ -93,6 +95,7 @@ struct FluxArgs {
   int tiles_per_pv;
   int64_t n_tiles;
   unsigned long long* sched;   // scheduler slot: [0] global tile ticket, [1] warps that have finished, [2+pv] per-pv tickets
+  const PvRec* pvcache;        // single passband, few parameter vectors: records precomputed by pv_cache_kernel (else NULL)
   int per_pv;                  // 1: warps stay on one parameter vector and take its tiles from sched[2+pv] (n_pv small)
   int lpt;                     // 1: global mode with the parameter vectors in order of decreasing expected work (n_pv <= kLptMax)
   // supersample accumulation (fixed point)
@@ -330,6 +333,22 @@ __device__ __noinline__ void tile_setup(const FluxArgs& A, WarpState& ws, int ri
       r.ob = kIsChi2<OutT> ? nullptr : (char*)A.flux + (pv * A.flux_pv_stride + A.flux_off + e0) * (int64_t)sizeof(OutT);
       r.e0 = e0;
       r.pv = pv;
+    }
+    __syncwarp();
+    return;
+  }
+  if (NPB1 && A.pvcache) {   // the record was computed once for the whole launch (pv_cache_kernel): copy, set the tile pointers
+    // programmatic dependent launch: this grid may have started while pv_cache_kernel was still running
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    const int64_t e0 = (int64_t)chunk * A.tile_len;
+    const double* src = reinterpret_cast<const double*>(A.pvcache + pv);
+    double* dst = reinterpret_cast<double*>(&r);
+    for (int i = lane; i < (int)(sizeof(PvRec) / sizeof(double)); i += 32) dst[i] = __ldg(src + i);
+    __syncwarp();
+    if (lane == 0) {
+      r.tb = A.times + pv * A.t_stride_pv + e0;
+      r.ob = kIsChi2<OutT> ? nullptr : (char*)A.flux + (pv * A.flux_pv_stride + A.flux_off + e0) * (int64_t)sizeof(OutT);
+      r.e0 = e0;
     }
     __syncwarp();
     return;
@@ -960,6 +979,23 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
       for (int64_t i = 0; i < nwords; ++i) A.sched[i] = 0ULL;
     }
   }
+}
+
+// Records of all parameter vectors, once per launch (single passband, few parameter vectors, many tiles each): a warp per
+// parameter vector runs the same setup the flux kernel would run per tile and stores the record to global memory; the
+// flux kernel then only copies it.  Raises the status flags (the flux kernel skips its own setup and with it the flags).
+template <int MODE>
+__global__ void __launch_bounds__(kThreads) pv_cache_kernel(const __grid_constant__ FluxArgs A, PvRec* __restrict__ out) {
+  __shared__ WarpState s_ws[kWarpsPerBlock];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  WarpState& ws = s_ws[warp];
+  asm volatile("griddepcontrol.launch_dependents;");   // the flux kernel may start launching: it waits before it reads
+  const int64_t pv = (int64_t)blockIdx.x * kWarpsPerBlock + warp;
+  if (pv >= A.n_pv) return;
+  tile_setup<MODE, true, double>(A, ws, 0, pv, 0, -1);
+  const double* src = reinterpret_cast<const double*>(&ws.pv[0]);
+  double* dst = reinterpret_cast<double*>(out + pv);
+  for (int i = lane; i < (int)(sizeof(PvRec) / sizeof(double)); i += 32) dst[i] = src[i];
 }
 
 }  // namespace pt

@@ -17,23 +17,28 @@ static std::atomic<int64_t> g_launches{0};
 // Scheduler slots of the flux kernel (tile counters + finished-warp counter each).  A launch takes the next slot in a ring;
 // the kernel leaves its slot zeroed when it ends, so a slot is clean again long before the ring comes back to it (that
 // would need kSchedSlots launches in flight at once).  This is the only state the library keeps on the device.
-constexpr int kSchedSlots = 1024;
+constexpr int kSchedSlots = 64;
 constexpr int kSchedWords = 1024;   // [0] global ticket, [1] finished warps, [2 + pv] per-parameter-vector tickets
-__device__ unsigned long long g_sched[kSchedSlots][kSchedWords];
+constexpr int kPvCacheMax = 512;    // parameter-vector records a slot can hold (pv_cache_kernel)
+struct SchedSlot {
+  unsigned long long w[kSchedWords];
+  PvRec pv[kPvCacheMax];
+};
+__device__ SchedSlot g_sched[kSchedSlots];
 static std::atomic<uint64_t> g_sched_seq{0};
 
-static unsigned long long* sched_slot() {
-  static std::atomic<unsigned long long*> base[64];
+static SchedSlot* sched_slot() {
+  static std::atomic<SchedSlot*> base[64];
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
-  unsigned long long* b = base[dev].load();
+  SchedSlot* b = base[dev].load();
   if (!b) {
     void* p = nullptr;
     if (cudaGetSymbolAddress(&p, g_sched) != cudaSuccess) return nullptr;
-    b = (unsigned long long*)p;
+    b = (SchedSlot*)p;
     base[dev].store(b);
   }
-  return b + (size_t)kSchedWords * (g_sched_seq.fetch_add(1) % kSchedSlots);
+  return b + (g_sched_seq.fetch_add(1) % kSchedSlots);
 }
 
 // S1-S2 alone: signed projected separation of every subsample.
@@ -231,8 +236,18 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   A.fx_inv = 1.0 / (A.fx_scale * (double)n_ss);
   A.inv_nss = 1.0 / (double)n_ss;
   const dim3 grid((unsigned)plan.blocks);
-  A.sched = sched_slot();
-  if (!A.sched) return PT_ERR_CUDA;
+  SchedSlot* slot = sched_slot();
+  if (!slot) return PT_ERR_CUDA;
+  A.sched = slot->w;
+  // single passband, few parameter vectors, many tiles each: the per-vector records are computed once, by a small kernel
+  // in front of the flux kernel (the setup is 15 % of the flux kernel's instructions on configs[1] when done per tile)
+  if (n_pb == 1 && pb_view < 0 && n_pv <= kPvCacheMax && A.n_tiles >= 8 * n_pv) {
+    const unsigned nb = (unsigned)((n_pv + kWarpsPerBlock - 1) / kWarpsPerBlock);
+    if (mode == 0) pv_cache_kernel<0><<<nb, kThreads, 0, st>>>(A, slot->pv);
+    else pv_cache_kernel<1><<<nb, kThreads, 0, st>>>(A, slot->pv);
+    A.pvcache = slot->pv;
+    g_launches.fetch_add(1);
+  }
   if (dtype == kDtypeChi2) {
     // step 1 of the fused likelihood: out-of-transit baseline into the tail of the scheduler slot, chi2[] zeroed
     double* part = reinterpret_cast<double*>(A.sched + kSchedWords - kBaseBlocks);
@@ -241,6 +256,7 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
     if (nb > kBaseBlocks) nb = kBaseBlocks;
     if (nb < 1) nb = 1;
     chi2_base_kernel<<<nb, kThreads, 0, st>>>(like->obs, like->isig, n_obs, part, (double*)d_flux, n_pv);
+    g_launches.fetch_add(1);
     A.obs = like->obs; A.isig = like->isig; A.chi2 = (double*)d_flux; A.base_part = part; A.n_base_part = nb;
     A.flux = nullptr;
   }
@@ -248,7 +264,15 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   const bool v2 = (n_t % 2 == 0) && (t_stride_pv % 2 == 0) && (reinterpret_cast<uintptr_t>(d_times) % 16 == 0) &&
                   (dtype == kDtypeChi2 || reinterpret_cast<uintptr_t>(d_flux) % 16 == 0);
   const bool p1 = (n_pb == 1), s1 = (n_ss == 1);
-#define PT_LAUNCH(M, VV, P, S, T) flux_kernel<M, VV, P, S, T><<<grid, kThreads, 0, st>>>(A)
+  // with the record cache the flux kernel is launched as a programmatic dependent of pv_cache_kernel: its launch and its
+  // prologue (row ranking) overlap that kernel, and it waits (griddepcontrol.wait) before it reads the first record
+  cudaLaunchAttribute pdl_attr[1];
+  pdl_attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  pdl_attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid; cfg.blockDim = dim3(kThreads); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+  cfg.attrs = pdl_attr; cfg.numAttrs = A.pvcache ? 1 : 0;
+#define PT_LAUNCH(M, VV, P, S, T) cudaLaunchKernelEx(&cfg, flux_kernel<M, VV, P, S, T>, A)
 #define PT_LAUNCH_S(M, VV, P, T)                             \
   do {                                                       \
     if (s1) PT_LAUNCH(M, VV, P, true, T);                    \
