@@ -37,7 +37,7 @@ ALG_PER_TRANSIT_ECC = 900.0   # the same with the Newton–Kepler solve
 FP64_LANES_PER_SM, N_SM = 64, 148
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/r1c_ncu_*.md);
 # a kernel's output that is still in L2 when the capture ends is not in its figure (configs[1]: 30.7 MB of flux < 126 MB L2).
-TRAFFIC_EXACT_CONFIG2 = 563.456e3 + 3.328e3
+TRAFFIC_EXACT_CONFIG2 = 572.416e3 + 10.496e3
 TRAFFIC_INTERP_F32 = 519.879936e6 + 3.233794e9
 TRAFFIC_DENSE = 134.598656e6 + 88.509696e6
 
