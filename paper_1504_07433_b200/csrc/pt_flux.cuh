@@ -754,7 +754,7 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
         const double P = row[1], a = row[2], ci = cos(row[3]), k = row[6 + 3 * A.pb_first];
         const double b = a * ci, c2 = (1.0 + k) * (1.0 + k) - b * b;
         float wgt = (float)(sqrt(fmax(c2, 0.0)) / (3.14159 * a) + ((A.n_ss > 1) ? fabs(A.t_exp / P) : 0.0));
-        if (!(wgt == wgt) || wgt > 1.0f) wgt = 1.0f;      // odd rows (bad parameters, a < 1+k): treat as heavy
+        if (!(wgt == wgt) || wgt > 1.0f || wgt < 0.0f) wgt = 1.0f;   // odd rows (bad parameters, a < 1+k): treat as heavy
         key = ((uint32_t)(wgt * 65535.0f) << 16) | (uint32_t)(0xffff - i);
       }
       s_key[i] = key;
