@@ -996,6 +996,9 @@ __global__ void __launch_bounds__(kThreads) pv_cache_kernel(const __grid_constan
   const double* src = reinterpret_cast<const double*>(&ws.pv[0]);
   double* dst = reinterpret_cast<double*>(out + pv);
   for (int i = lane; i < (int)(sizeof(PvRec) / sizeof(double)); i += 32) dst[i] = src[i];
+  // when this kernel was itself launched as a programmatic dependent (fused likelihood: of chi2_base_kernel), its
+  // completion must imply that kernel's: the flux kernel waits for this one only
+  asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
 }  // namespace pt

@@ -106,6 +106,7 @@ __global__ void __launch_bounds__(kThreads) chi2_base_kernel(const double* __res
                                                              int64_t n, double* __restrict__ part, double* __restrict__ chi2,
                                                              int64_t n_pv) {
   __shared__ double s_sum[kThreads];
+  asm volatile("griddepcontrol.launch_dependents;");   // the record kernel does not read this kernel's output
   const int64_t per = (n + gridDim.x - 1) / gridDim.x;
   const int64_t lo = (int64_t)blockIdx.x * per, hi = min(lo + per, n);
   double acc = 0.0;
@@ -243,8 +244,16 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   // in front of the flux kernel (the setup is 15 % of the flux kernel's instructions on configs[1] when done per tile)
   if (n_pb == 1 && pb_view < 0 && n_pv <= kPvCacheMax && A.n_tiles >= 8 * n_pv) {
     const unsigned nb = (unsigned)((n_pv + kWarpsPerBlock - 1) / kWarpsPerBlock);
-    if (mode == 0) pv_cache_kernel<0><<<nb, kThreads, 0, st>>>(A, slot->pv);
-    else pv_cache_kernel<1><<<nb, kThreads, 0, st>>>(A, slot->pv);
+    // fused likelihood: the record kernel overlaps chi2_base_kernel (it waits for it only before it exits, so that the
+    // flux kernel, which waits for the record kernel, also sees the baseline)
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchConfig_t c2{};
+    c2.gridDim = dim3(nb); c2.blockDim = dim3(kThreads); c2.dynamicSmemBytes = 0; c2.stream = st;
+    c2.attrs = at; c2.numAttrs = (dtype == kDtypeChi2) ? 1 : 0;
+    if (mode == 0) cudaLaunchKernelEx(&c2, pv_cache_kernel<0>, A, slot->pv);
+    else cudaLaunchKernelEx(&c2, pv_cache_kernel<1>, A, slot->pv);
     A.pvcache = slot->pv;
     g_launches.fetch_add(1);
   }
