@@ -534,4 +534,17 @@ int pto_ma_quad_interp(int prec, const void* table, int32_t table_dtype, int32_t
                    : flux_impl<quad>(1, &tb, times, n_t, t_stride_pv, params, n_pv, n_pb, n_ss, t_exp, flux_out);
 }
 
+// bilinear rule alone at n (k,z) pairs (pins the cell choice and the clamps of interp_basis); out[n][3]
+int pto_interp_basis(int prec, const void* table, int32_t table_dtype, int32_t n_k, int32_t n_z, int32_t n_fn, double k_min,
+                     double dk, double dz, const double* k, const double* z, int64_t n, double* out) {
+  if (!table || !k || !z || !out) return 1;
+  if (n_k < 2 || n_z < 2 || (n_fn != 3 && n_fn != 4) || !(dk > 0.0) || !(dz > 0.0)) return 4;
+  TableView tb{table, table_dtype, n_k, n_z, n_fn, k_min, dk, dz};
+  for (int64_t i = 0; i < n; ++i) {
+    if (prec == 0) { double v[3]; interp_basis<double>(tb, k[i], z[i], v); for (int f = 0; f < 3; ++f) out[3 * i + f] = v[f]; }
+    else { quad v[3]; interp_basis<quad>(tb, quad(k[i]), quad(z[i]), v); for (int f = 0; f < 3; ++f) out[3 * i + f] = (double)v[f]; }
+  }
+  return 0;
+}
+
 }  // extern "C"

@@ -41,7 +41,7 @@ def lib() -> C.CDLL:
         if _lib is None:
             _lib = C.CDLL(build())
             for name in ("pto_ma_basis", "pto_ellip", "pto_kepler", "pto_orbit_z", "pto_ma_quad_exact",
-                         "pto_ma_table_build", "pto_ma_quad_interp", "pto_num_threads"):
+                         "pto_ma_table_build", "pto_ma_quad_interp", "pto_interp_basis", "pto_num_threads"):
                 getattr(_lib, name).restype = C.c_int
             _lib.pto_set_num_threads.restype = None
     return _lib
@@ -157,6 +157,21 @@ def ma_quad_interp(table, k_min, dk, dz, times, params, n_pb: int = 1, n_ss: int
                                   C.c_int32(n_ss), C.c_double(t_exp), _p(f))
     assert rc == 0, rc
     return f
+
+
+def interp_basis(table, k_min, dk, dz, k, z, prec: str = "f128"):
+    """The bilinear rule alone (S§8(c)-2 step 8): λe, λd*, ηd [n][3] looked up in `table` at (k, z)."""
+    table = np.ascontiguousarray(table)
+    code = {np.dtype(np.float64): 0, np.dtype(np.float32): 1}[table.dtype]
+    n_k, n_z, n_fn = table.shape
+    k, z = np.broadcast_arrays(_f64(k), _f64(z))
+    k, z = _f64(k), _f64(z)
+    out = np.empty((k.size, 3), np.float64)
+    rc = lib().pto_interp_basis(C.c_int(PREC[prec]), _p(table), C.c_int32(code), C.c_int32(n_k), C.c_int32(n_z),
+                                C.c_int32(n_fn), C.c_double(k_min), C.c_double(dk), C.c_double(dz), _p(k), _p(z),
+                                C.c_int64(k.size), _p(out))
+    assert rc == 0, rc
+    return out.reshape(k.shape + (3,))
 
 
 def chi2_of_flux(flux, obs, isig):

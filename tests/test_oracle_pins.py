@@ -327,6 +327,47 @@ def test_bilinear_rule_reproduces_an_affine_table(oracle):
         assert np.abs(f[pv, 0] - ref).max() <= 1e-14
 
 
+
+def test_bilinear_cell_choice_on_a_non_affine_table(oracle):
+    """Cell choice and clamps of the bilinear rule (S§8(c)-2 step 8) on a table that is NOT affine, so a
+    wrong cell (ceil/round instead of floor, a shifted clamp, swapped k/z weights) changes the value: expected values are
+    numpy.interp along z in each of the two bracketing k-rows, blended linearly in k."""
+    k_min, dk, n_k, dz, n_z = 0.05, 0.0125, 17, 0.03125, 41          # dk, dz exactly representable: nodes are exact
+    kk = k_min + np.arange(n_k) * dk
+    zz = np.arange(n_z) * dz
+    K, Z = np.meshgrid(kk, zz, indexing="ij")
+    tb = np.stack([Z * Z + 0.1 * K, np.sin(3.0 * Z) + K * K, K * np.exp(Z)], axis=2)
+    z_max = zz[-1]
+    rng = np.random.default_rng(5)
+    kq = np.concatenate([rng.uniform(k_min, kk[-1], 400), kk[[0, 3, 16]], [kk[3] + 0.25 * dk, kk[15] + 0.999 * dk]])
+    zq = np.concatenate([rng.uniform(0.0, z_max, 380), zz[[0, 1, 7, 39, 40]], zz[7] + dz * np.array([1e-9, 0.5, 1 - 1e-9]),
+                         z_max - dz * np.array([0.75, 0.5, 1e-12]), [z_max + 0.01, z_max + 0.3, 0.0],  # last cell; beyond z_max
+                         rng.uniform(0.0, z_max, 11)])
+    assert kq.size == zq.size
+    got = oracle.interp_basis(tb, k_min, dk, dz, kq, zq, prec="f128")
+    ik = np.minimum(np.floor((kq - k_min) / dk).astype(int), n_k - 2)
+    fk = (kq - k_min) / dk - ik
+    for f in range(3):
+        lo = np.array([np.interp(min(z, z_max), zz, tb[i, :, f]) for i, z in zip(ik, zq)])
+        hi = np.array([np.interp(min(z, z_max), zz, tb[i + 1, :, f]) for i, z in zip(ik, zq)])
+        inside = zq <= z_max
+        ref = (1 - fk) * lo + fk * hi
+        assert np.abs(got[inside, f] - ref[inside]).max() <= 1e-14
+    # beyond z_max the clamp keeps the LAST cell and extrapolates along its segment (iz = n_z-2, fz > 1)
+    out = zq > z_max
+    for f in range(3):
+        seg = lambda i, z: tb[i, -2, f] + (z - zz[-2]) / dz * (tb[i, -1, f] - tb[i, -2, f])
+        ref = np.array([(1 - w) * seg(i, z) + w * seg(i + 1, z) for i, w, z in zip(ik[out], fk[out], zq[out])])
+        assert np.abs(got[out, f] - ref).max() <= 1e-13
+    # exactly on a node the node value comes back (k on a node and z on a node)
+    g = oracle.interp_basis(tb, k_min, dk, dz, np.repeat(kk[[0, 5, 16]], 3), np.tile(zz[[0, 9, 40]], 3))
+    assert np.abs(g - tb[np.repeat([0, 5, 16], 3), np.tile([0, 9, 40], 3)]).max() <= 1e-15
+    # an fp32-stored table is converted on load, the arithmetic stays in the working precision
+    g32 = oracle.interp_basis(tb.astype(np.float32), k_min, dk, dz, kq[:50], zq[:50])
+    g64 = oracle.interp_basis(tb.astype(np.float32).astype(np.float64), k_min, dk, dz, kq[:50], zq[:50])
+    assert np.array_equal(g32, g64)
+
+
 def test_p11_paper_interpolation_error_figures(oracle):
     """P:L149: default table n_k=128, n_z=256, Δk=0.02: max error ~4 ppm, mean over the transit ~0.05 ppm;
     P:L216: the maximum sits at the end of ingress / start of egress.  Order-of-magnitude check (the paper does not
