@@ -103,7 +103,8 @@ def config3(n_pv: int = 512, n_pb: int = 20, n_t: int = 600, stream: int = 0) ->
     head = np.stack([t0, P, a, inc, z, z], axis=1)
     tail = np.stack([k, u1, u2], axis=2).reshape(n_pv, 3 * n_pb)
     params = np.concatenate([head, tail], axis=1)
-    times = -0.12 + 0.24 * np.arange(n_t, dtype=np.float64) / (n_t - 1)
+    # a single exposure sits at mid-transit (0/0 otherwise)
+    times = -0.12 + 0.24 * np.arange(n_t, dtype=np.float64) / (n_t - 1) if n_t > 1 else np.zeros(1)
     return Workload("config3", times, params, n_pb=n_pb)
 
 
