@@ -318,7 +318,7 @@ def run_ours(args):
             co = torch.empty(wl.n_pv, dtype=torch.float64, device=dev)
             t_c = _time_steps(lambda: pt.pt_ma_quad_chi2(ct, cp, obs, isig, 1, wl.n_ss, wl.t_exp, table=tbl, out=co),
                               10, 3, flush, 1) / 10
-            res_c[name] = {"value": wl.n_eval / t_c, "unit": UNIT, "ms": t_c * 1e3, "launches_per_call": 2 if wl.n_pv > 512 else 3}
+            res_c[name] = {"value": wl.n_eval / t_c, "unit": UNIT, "ms": t_c * 1e3, "launches_per_call": 2}
             del ct, cp, obs, isig, co, tbl
         res_c["note"] = ("pt_ma_quad_chi2: chi2[pv] against one data set; out-of-window exposures cost a window test and no "
                          "memory traffic (times are L2-resident), so the flux-store roofline does not apply")

@@ -97,6 +97,10 @@ int pt_ma_quad_exact_pbk(const double* d_times, int64_t n_t, int64_t t_stride_pv
 int pt_ma_table_build(double k_min, double k_max, int32_t n_k, double z_max, int32_t n_z, int32_t dtype, int32_t n_fn,
                       void* d_table, void* stream);
 
+/* Node spacing of the table pt_ma_table_build builds for these arguments, exactly as the builder forms it in IEEE double:
+ * *h_dk = (k_max-k_min)/(n_k-1), *h_dz = z_max/(n_z-1).  Host pointers; this is what belongs in pt_table.dk / .dz. */
+int pt_table_spacing(double k_min, double k_max, int32_t n_k, double z_max, int32_t n_z, double* h_dk, double* h_dz);
+
 /* S9 (+S0-S3, S6, S7): interpolated quadratic Mandel–Agol flux ("bilinear interpolation"):
  *   rk = (k̂-k_min)/dk, ik = min(floor(rk), n_k-2), fk = rk-ik; rz = z/dz, iz = min(floor(rz), n_z-2), fz = rz-iz;
  *   v = (1-fk)[(1-fz)T[ik][iz] + fz T[ik][iz+1]] + fk[(1-fz)T[ik+1][iz] + fz T[ik+1][iz+1]] for each function, then

@@ -20,7 +20,7 @@ PT_F64, PT_F32 = 0, 1
 PT_ST_BAD_PARAM, PT_ST_K_OUT_OF_TABLE = 1, 2
 _ERR = {1: "PT_ERR_NULL", 2: "PT_ERR_SIZE", 3: "PT_ERR_DTYPE", 4: "PT_ERR_TABLE", 5: "PT_ERR_CUDA"}
 
-EXPORTS = ("pt_build_arch", "pt_orbit_z", "pt_ma_quad_exact", "pt_ma_table_build", "pt_ma_quad_interp", "pt_ma_quad_chi2", "pt_ma_quad_exact_pbk",
+EXPORTS = ("pt_build_arch", "pt_orbit_z", "pt_ma_quad_exact", "pt_ma_table_build", "pt_table_spacing", "pt_ma_quad_interp", "pt_ma_quad_chi2", "pt_ma_quad_exact_pbk",
            "pt_ma_quad_exact_host", "pt_ma_quad_interp_host", "pt_plan", "pt_probe_dfma", "pt_launch_count")
 
 
@@ -52,6 +52,7 @@ def lib() -> C.CDLL:
         L.pt_ma_quad_exact.argtypes = common + [i32, ptr, ptr, ptr]
         L.pt_ma_quad_exact_pbk.argtypes = common + [i32, ptr, ptr, ptr]
         L.pt_ma_table_build.argtypes = [dbl, dbl, i32, dbl, i32, i32, i32, ptr, ptr]
+        L.pt_table_spacing.argtypes = [dbl, dbl, i32, dbl, i32, C.POINTER(dbl), C.POINTER(dbl)]
         L.pt_ma_quad_interp.argtypes = [C.POINTER(pt_table)] + common + [i32, ptr, ptr, ptr]
         L.pt_ma_quad_chi2.argtypes = [C.POINTER(pt_table), ptr, i64, ptr, i64, i32, i32, dbl, ptr, ptr, ptr, ptr, ptr]
         L.pt_ma_quad_exact_host.argtypes = common + [i32, ptr, ptr]
@@ -157,9 +158,10 @@ def pt_ma_table_build(k_min: float, k_max: float, n_k: int, z_max: float, n_z: i
     data = torch.empty((n_k, n_z, n_fn), dtype=dtype, device=device)
     _check(lib().pt_ma_table_build(float(k_min), float(k_max), n_k, float(z_max), n_z, _dtype_code(dtype), n_fn,
                                    data.data_ptr(), _stream()), "pt_ma_table_build")
-    dk = (float(k_max) - float(k_min)) / float(n_k - 1)
-    dz = float(z_max) / float(n_z - 1)
-    return Table(data, k_min, dk, dz)
+    dk, dz = C.c_double(), C.c_double()
+    _check(lib().pt_table_spacing(float(k_min), float(k_max), n_k, float(z_max), n_z, C.byref(dk), C.byref(dz)),
+           "pt_table_spacing")
+    return Table(data, k_min, dk.value, dz.value)
 
 
 def pt_ma_quad_interp(table: Table, times: torch.Tensor, params: torch.Tensor, n_pb: int = 1, n_ss: int = 1,

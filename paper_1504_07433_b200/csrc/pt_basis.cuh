@@ -166,7 +166,10 @@ __device__ __forceinline__ Basis ma_basis(double p, double z) {
       }
     }
   }
-  r.ld = fma(pref, cel_pair(mc, sp, cK, cE, cP, a2, b2), add);
+  // λd* is the integral of a non-negative function: close to the outer contact, where its O(1) elliptic-integral terms
+  // cancel down to less than their rounding error (a few 1e-16), the sum can come out negative — clamped, so that a
+  // physical limb-darkening law never yields a flux above 1
+  r.ld = fmax(fma(pref, cel_pair(mc, sp, cK, cE, cP, a2, b2), add), 0.0);
   return r;
 }
 

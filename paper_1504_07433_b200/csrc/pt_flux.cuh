@@ -52,7 +52,8 @@ constexpr int kPvRing = 4;      // parameter-vector records a warp keeps alive (
 constexpr int kCoefCache = 32;  // passbands whose combine coefficients are cached per warp (multi-passband path)
 constexpr int kMaxTileLen = 32768;
 constexpr int kRemBias = 1 << 24;
-constexpr int kLptMax = 512;    // parameter vectors that the longest-processing-time-first order is built for
+constexpr int kSchedHead = 8;   // words of a scheduler slot in front of the per-parameter-vector tickets
+constexpr unsigned long long kSlotUnsorted = 1ULL;   // flag word: the shared time axis is not ascending / not finite
 // -DPT_DEBUG_CHECKS: capacity invariants of the per-warp queues are checked and a violation traps (the test suite is run
 // once against such a build; compute-sanitizer is not available on the GPU pool).
 #ifdef PT_DEBUG_CHECKS
@@ -94,10 +95,15 @@ struct FluxArgs {
   int tile_len;            // exposures per tile (multiple of 256, <= kMaxTileLen)
   int tiles_per_pv;
   int64_t n_tiles;
-  unsigned long long* sched;   // scheduler slot: [0] global tile ticket, [1] warps that have finished, [2+pv] per-pv tickets
-  const PvRec* pvcache;        // single passband, few parameter vectors: records precomputed by pv_cache_kernel (else NULL)
-  int per_pv;                  // 1: warps stay on one parameter vector and take its tiles from sched[2+pv] (n_pv small)
-  int lpt;                     // 1: global mode with the parameter vectors in order of decreasing expected work (n_pv <= kLptMax)
+  unsigned long long* sched;   // scheduler slot: [0] global tile ticket, [1] warps that have finished, [2] flags (kSlotUnsorted),
+                               // [kSchedHead + pv] per-pv tickets
+  const PvRec* pvcache;        // single passband, few parameter vectors: records precomputed by prep_kernel (else NULL)
+  const uint32_t* order;       // global mode: row order of the tiles written by prep_kernel (heaviest rows first / rows sorted
+                               // by k̂ for the table), or NULL = index order
+  int per_pv;                  // 1: warps stay on one parameter vector and take its tiles from its own counter (n_pv small)
+  int prep;                    // 1: launched as a programmatic dependent of prep_kernel: wait for it before reading the slot
+  int range;                   // 1: one shared time axis; if prep_kernel found it ascending and finite, out-of-window
+                               // stretches are found by search and written as pure fills (no per-exposure window test)
   // supersample accumulation (fixed point)
   int fx_bits;             // 61 - ceil(log2 n_ss): a sum of n_ss values below 2^eb fits an int64 at scale 2^(fx_bits-eb)
   double fx_scale;         // 2^fx_bits (basis values are <= 1)
@@ -106,7 +112,7 @@ struct FluxArgs {
   // interpolation table (mode 1)
   const void* tb;
   int tb_dtype, n_k, n_z, n_fn;
-  double k_min, dk, dz;
+  double k_min, dk, dz, inv_dz;
 };
 
 __device__ __forceinline__ double nan64() { return __longlong_as_double(0x7ff8000000000000LL); }
@@ -136,7 +142,16 @@ struct Slot {              // a supersampled exposure with subsamples still in t
   uint16_t ring;           // PvRec index
 };
 
+// Range mode (ascending shared time axis): the transit epochs of the current tile that are still to be looked at, and the
+// current batch of up to 32 of them — exposures [lo[i], hi[i]) of the tile can be in transit at epoch i of the batch.
+struct RangeState {
+  double n, nend;          // next epoch, last epoch (n > nend: none left)
+  double T0, idt;          // first time of the tile, (n_e - 1) / (last - first): the search's first guess
+  int lo[32], hi[32];
+};
+
 struct WarpState {
+  RangeState rg;
   PvRec pv[kPvRing];
   uint16_t expq[kExpQ];
   double coefc[3 * kCoefCache];
@@ -266,7 +281,7 @@ __device__ __forceinline__ float4 ldg_keep4(const float* p, unsigned long long p
 template <typename TT>
 __device__ __forceinline__ Basis table_lookup(const FluxArgs& A, int ik, double fk, double z) {
   const unsigned long long pol = l2_keep_policy();
-  const double rz = z / A.dz;
+  const double rz = z * A.inv_dz;     // 1 ulp from z/dz: moves fz by 1e-16 rz, the value by < 1e-16 (bilinear is continuous across cells)
   int iz = (int)floor(rz);
   iz = min(max(iz, 0), A.n_z - 2);
   const double fz = rz - (double)iz;
@@ -337,9 +352,7 @@ __device__ __noinline__ void tile_setup(const FluxArgs& A, WarpState& ws, int ri
     __syncwarp();
     return;
   }
-  if (NPB1 && A.pvcache) {   // the record was computed once for the whole launch (pv_cache_kernel): copy, set the tile pointers
-    // programmatic dependent launch: this grid may have started while pv_cache_kernel was still running
-    asm volatile("griddepcontrol.wait;" ::: "memory");
+  if (NPB1 && A.pvcache) {   // the record was computed once for the whole launch (prep_kernel): copy, set the tile pointers
     const int64_t e0 = (int64_t)chunk * A.tile_len;
     const double* src = reinterpret_cast<const double*>(A.pvcache + pv);
     double* dst = reinterpret_cast<double*>(&r);
@@ -683,14 +696,14 @@ __device__ __forceinline__ bool next_pv(const FluxArgs& A, int64_t& pv, int& chu
   for (int64_t off = 1; off < n_pv; off += 32) {
     const int64_t cand = (pv + off + lane) % n_pv;
     const bool in_range = off + lane < n_pv;
-    const unsigned long long seen = in_range ? *((volatile unsigned long long*)(A.sched + 2 + cand)) : tpp;
+    const unsigned long long seen = in_range ? *((volatile unsigned long long*)(A.sched + kSchedHead + cand)) : tpp;
     unsigned avail = __ballot_sync(0xffffffffu, seen < tpp);
     while (avail) {
       const int src = __ffs(avail) - 1;
       avail &= avail - 1u;
       const int64_t target = (pv + off + src) % n_pv;
       unsigned long long got = 0;
-      if (lane == 0) got = atomicAdd(A.sched + 2 + target, 1ULL);
+      if (lane == 0) got = atomicAdd(A.sched + kSchedHead + target, 1ULL);
       got = __shfl_sync(0xffffffffu, got, 0);
       if (got < tpp) {
         pv = target;
@@ -700,6 +713,82 @@ __device__ __forceinline__ bool next_pv(const FluxArgs& A, int64_t& pv, int& chu
     }
   }
   return false;
+}
+
+// flux = 1 for exposures [a, b) of the tile, all passbands: the out-of-transit stretches of range mode.  V == 2: a and b
+// are even and the rows 16-byte aligned, every lane stores aligned pairs; 512 contiguous bytes per warp instruction.
+template <int V, bool NPB1, typename OutT>
+__device__ __forceinline__ void fill_ones(OutT* __restrict__ ob, uint32_t a, uint32_t b, int64_t n_t, int n_pb) {
+  if constexpr (kIsChi2<OutT>) {
+    return;   // flux 1 is what the chi2 baseline assumes
+  } else {
+    const uint32_t lane = threadIdx.x & 31;
+    const int np = NPB1 ? 1 : n_pb;
+    const uint32_t n = b - a;                       // warp-uniform: the trip count is too, only the tail is predicated
+    for (int j = 0; j < np; ++j) {
+      if (V == 2) {
+        typedef typename Vec2<OutT>::type V2;
+        V2 v;
+        v.x = (OutT)1.0; v.y = (OutT)1.0;
+        V2* p = (V2*)(ob + (int64_t)j * n_t + a) + lane;
+#pragma unroll 4
+        for (uint32_t i = n >> 6; i > 0; --i) { PT_ST(p, v); p += 32; }
+        if (2u * lane < (n & 63u)) PT_ST(p, v);
+      } else {
+        OutT* p = ob + (int64_t)j * n_t + a + lane;
+#pragma unroll 4
+        for (uint32_t i = n >> 5; i > 0; --i) { PT_ST(p, (OutT)1.0); p += 32; }
+        if (lane < (n & 31u)) PT_ST(p, (OutT)1.0);
+      }
+    }
+  }
+}
+
+// First index i in [0, n] with t[i] >= x (STRICT = false) or t[i] > x (STRICT = true) in the ascending array t[0..n),
+// given four consecutive values v[0..3] = t[s..s+3] that were loaded around the index a uniform cadence predicts (the
+// caller issues those loads for both ends of a range at once: one memory latency per batch of epochs).  If the answer is
+// not bracketed by the probe (an unevenly sampled axis), gallop outwards from it and bisect: O(log n) for any ascending axis.
+template <bool STRICT>
+__device__ __forceinline__ int search_sorted(const double* __restrict__ t, int n, double x, int s, const double (&v)[4]) {
+  int c = 0;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) c += (STRICT ? v[i] <= x : v[i] < x) ? 1 : 0;
+  if ((c > 0 || s == 0) && (c < 4 || s + 4 >= n)) return min(s + c, n);
+  int lo, hi;
+  if (c == 0) {                      // the answer is < s: gallop down
+    hi = s;
+    lo = s - 1;
+    int step = 1;
+    while (lo >= 0) {
+      const double w = __ldg(t + lo);
+      if (STRICT ? w <= x : w < x) break;
+      hi = lo; lo -= step; step <<= 1;
+    }
+    lo = max(lo, -1) + 1;
+  } else {                           // the answer is > s + 3: gallop up
+    lo = s + 4;
+    hi = s + 4;
+    int step = 1;
+    while (hi < n) {
+      const double w = __ldg(t + hi);
+      if (!(STRICT ? w <= x : w < x)) break;
+      lo = hi + 1; hi += step; step <<= 1;
+    }
+    hi = min(hi, n);
+  }
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    const double w = __ldg(t + mid);
+    if (STRICT ? w <= x : w < x) lo = mid + 1; else hi = mid;
+  }
+  return lo;
+}
+// Start of the four-value probe for x: one below the index a uniform cadence predicts, clamped so that s..s+3 is in range
+// (n >= 4; shorter tiles never take range mode).
+__device__ __forceinline__ int probe_start(double x, int n, double T0, double idt) {
+  const double gf = (x - T0) * idt;
+  const int g = gf > 1.0 ? (gf < (double)(n - 1) ? (int)gf : n - 1) : 1;
+  return min(g - 1, n - 4);
 }
 
 // ---------------------------------------------------------------------------------------------------- the kernel
@@ -739,51 +828,12 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
   //     parameter vector (setup done once, later tiles only move the tile pointers) and moves on to the next one that has
   //     tiles left when it is exhausted, so fast parameter vectors lend their warps to slow ones.
   // The last warp to finish zeroes the slot for the next launch that uses it.
-  // LPT order: tiles of rows with many (long) transits are dealt first, so that the launch ends on light tiles.  The
-  // expected work of a row is its in-window fraction, roughly sqrt((1+k)² - b²) / (π a) + t_exp / P; the estimate only
-  // orders the tiles.  One block barrier, before any warp starts its pipeline.
-  __shared__ uint32_t s_key[kLptMax];      // (quantised weight << 16) | (0xffff - row): unique keys, sorted descending
-  if (A.lpt) {
-    const int n = (int)A.n_pv;
-    int np2 = 32;
-    while (np2 < n) np2 <<= 1;
-    for (int i = threadIdx.x; i < np2; i += kThreads) {
-      uint32_t key = 0u;                                  // padding sorts last
-      if (i < n) {
-        const double* row = A.params + (int64_t)i * A.row_stride;
-        const double P = row[1], a = row[2], ci = cos(row[3]), k = row[6 + 3 * A.pb_first];
-        const double b = a * ci, c2 = (1.0 + k) * (1.0 + k) - b * b;
-        float wgt = (float)(sqrt(fmax(c2, 0.0)) / (3.14159 * a) + ((A.n_ss > 1) ? fabs(A.t_exp / P) : 0.0));
-        if (!(wgt == wgt) || wgt > 1.0f || wgt < 0.0f) wgt = 1.0f;   // odd rows (bad parameters, a < 1+k): treat as heavy
-        key = ((uint32_t)(wgt * 65535.0f) << 16) | (uint32_t)(0xffff - i);
-      }
-      s_key[i] = key;
-    }
-    __syncthreads();
-    if (n <= 128) {                                       // few rows: rank by counting (one more barrier instead of ~28)
-      uint32_t mine = 0u;
-      int rank = 0;
-      if ((int)threadIdx.x < n) {
-        mine = s_key[threadIdx.x];
-        for (int j = 0; j < n; ++j) rank += (s_key[j] > mine) ? 1 : 0;
-      }
-      __syncthreads();
-      if ((int)threadIdx.x < n) s_key[rank] = mine;
-      __syncthreads();
-    } else
-    for (int size = 2; size <= np2; size <<= 1) {         // bitonic sort, descending
-      for (int stride = size >> 1; stride > 0; stride >>= 1) {
-        for (int t = threadIdx.x; t < (np2 >> 1); t += kThreads) {
-          const int lo = 2 * t - (t & (stride - 1));
-          const int hi = lo + stride;
-          const bool desc = (lo & size) == 0;
-          const uint32_t x = s_key[lo], y = s_key[hi];
-          if ((x < y) == desc) { s_key[lo] = y; s_key[hi] = x; }
-        }
-        __syncthreads();
-      }
-    }
-  }
+  // Row order of the tiles (global mode): prep_kernel ranks the rows — by decreasing expected in-window fraction for the
+  // exact model (longest processing time first: the launch ends on light tiles), by k̂ for the interpolated model (tiles
+  // in flight then share a few k-rows of the table, which stay in L1/L2 while gigabytes of flux stream past).
+  // The slot (order, records, flags) is written by prep_kernel, whose programmatic dependent this grid is.
+  if (A.prep) asm volatile("griddepcontrol.wait;" ::: "memory");
+  const bool sorted_axis = A.range && !(*((volatile const unsigned long long*)(A.sched + 2)) & kSlotUnsorted);
   const int tpp = A.tiles_per_pv;
   int64_t pv_cur = 0, last_pv = -1;
   int chunk_cur = 0, last_ring = -1;
@@ -792,11 +842,11 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
     have = gw < A.n_tiles;
     pv_cur = gw / tpp;
     chunk_cur = (int)(gw - pv_cur * tpp);
-    if (A.lpt && have) pv_cur = 0xffff - (int)(s_key[pv_cur] & 0xffffu);
+    if (A.order && have) pv_cur = (int64_t)__ldg(A.order + pv_cur);
   } else {
     pv_cur = gw % A.n_pv;
     unsigned long long f0 = 0;
-    if (lane == 0) f0 = atomicAdd(A.sched + 2 + pv_cur, 1ULL);
+    if (lane == 0) f0 = atomicAdd(A.sched + kSchedHead + pv_cur, 1ULL);
     f0 = __shfl_sync(0xffffffffu, f0, 0);
     have = f0 < (unsigned long long)tpp;
     chunk_cur = (int)f0;
@@ -813,6 +863,9 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
   int ms0 = 0, msid = -1;        // n_ss > 32: sub-round state of the exposure being expanded
   double chi_acc = 0.0;          // fused likelihood, n_ss == 1: this lane's chi2 corrections of the current tile
   uint32_t base = 0, n_e = 0;
+  // range mode: position in / size of the current batch of epochs (the rest of the state lives in ws.rg)
+  bool rng_on = false;
+  int rng_i = 0, rng_cnt = 0;
   unsigned long long fetched = 0;
   const double* __restrict__ tb = nullptr;
   OutT* __restrict__ ob = nullptr;
@@ -851,13 +904,66 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
           have = tile < A.n_tiles;
           pv_cur = tile / tpp;
           chunk_cur = (int)(tile - pv_cur * tpp);
-          if (A.lpt && have) pv_cur = 0xffff - (int)(s_key[pv_cur] & 0xffffu);
+          if (A.order && have) pv_cur = (int64_t)__ldg(A.order + pv_cur);
         } else if (nf < (unsigned long long)tpp) {
           chunk_cur = (int)nf;
         } else {
           have = next_pv(A, pv_cur, chunk_cur);
         }
         phase = have ? PH_NEWTILE : PH_EXIT;
+        continue;
+      }
+      if (rng_on) {
+        // ---- range mode: exposures between the in-window ranges are pure fills (no time loads, no arithmetic)
+        const PvRec& r = ws.pv[C.cur];
+        do {
+          if (rng_i == rng_cnt) {
+            const double n0 = ws.rg.n, nend = ws.rg.nend;
+            if (!(n0 <= nend)) {                                   // no epoch left: the rest of the tile is out of transit
+              fill_ones<V, NPB1, OutT>(ob, base, n_e, A.n_t, n_pb);
+              base = n_e;
+              break;
+            }
+            // next batch of epochs, one per lane: [t0 + (n + ex_lo) P, t0 + (n + ex_hi) P] widened by the rounding of this
+            // very expression (ex_lo/ex_hi already carry the 1e-7-cycle margin of the window, pt_orbit.cuh)
+            const double n = n0 + (double)lane;
+            int lo = (int)n_e, hi = (int)n_e;
+            if (n <= nend) {
+              const double padn = 0x1p-49 * (fabs(n) + fabs(r.c.t0 * r.c.invP) + 1.0);
+              const double tlo = fma(r.c.P, n + (r.c.ex_lo - padn), r.c.t0);
+              const double thi = fma(r.c.P, n + (r.c.ex_hi + padn), r.c.t0);
+              const double T0 = ws.rg.T0, idt = ws.rg.idt;
+              const int sl = probe_start(tlo, (int)n_e, T0, idt), sh = probe_start(thi, (int)n_e, T0, idt);
+              double vl[4], vh[4];
+#pragma unroll
+              for (int i = 0; i < 4; ++i) { vl[i] = __ldg(tb + sl + i); vh[i] = __ldg(tb + sh + i); }   // 8 independent loads
+              lo = search_sorted<false>(tb, (int)n_e, tlo, sl, vl) & ~(V - 1);
+              hi = min((search_sorted<true>(tb, (int)n_e, thi, sh, vh) + (V - 1)) & ~(V - 1), (int)n_e);
+            }
+            __syncwarp();
+            ws.rg.lo[lane] = lo; ws.rg.hi[lane] = hi;
+            if (lane == 0) ws.rg.n = n0 + 32.0;
+            __syncwarp();
+            const double left = nend - n0 + 1.0;
+            rng_cnt = left < 32.0 ? (int)left : 32;
+            rng_i = 0;
+          }
+          const int lo = max(ws.rg.lo[rng_i], (int)base);
+          const int hi = ws.rg.hi[rng_i];
+          if (hi <= lo) { ++rng_i; continue; }                     // no exposure at this epoch (or swallowed by the previous range)
+          fill_ones<V, NPB1, OutT>(ob, base, (uint32_t)lo, A.n_t, n_pb);
+          const int cnt = min(hi - lo, 32);
+          if (lane < cnt) {
+            ws.expq[(C.qhead + C.qcount + lane) & (kExpQ - 1)] = (uint16_t)(lo + lane);
+            if ((lane & 15) == 0) asm volatile("prefetch.global.L1 [%0];" ::"l"(tb + lo + lane));   // times the z-round reads next
+          }
+          __syncwarp();
+          C.qcount += cnt;
+          PT_CHECK(C.qcount <= kExpQ);
+          base = (uint32_t)(lo + cnt);
+          if ((int)base >= hi) ++rng_i;
+        } while (C.qcount < EPW);
+        if (base >= n_e) keep = 1;
         continue;
       }
       // ---- stream super-groups of kUnroll x 32 lanes x V exposures until a z-round is due or the tile ends
@@ -936,7 +1042,7 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
         if (clash) { drain_all = true; continue; }
       }
       fetched = 0;
-      if (lane == 0) fetched = atomicAdd(A.per_pv ? A.sched + 2 + pv_cur : A.sched, 1ULL);
+      if (lane == 0) fetched = atomicAdd(A.per_pv ? A.sched + kSchedHead + pv_cur : A.sched, 1ULL);
       tile_setup<MODE, NPB1, OutT>(A, ws, ring, pv_cur, chunk_cur, (pv_cur == last_pv) ? last_ring : -1);
       last_pv = pv_cur;
       last_ring = ring;
@@ -965,6 +1071,30 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
         if (lane == 0) atomicAdd(A.chi2 + pv_cur, b);
       }
       w_invP = r.c.invP; w_c0 = r.w_c0; w_half = r.w_half;
+      // range mode for this tile?  Needs the ascending axis and no more transit epochs than a few per hundred exposures
+      // (else the per-exposure window test is the cheaper way); a row that is always in the window streams as before
+      rng_on = false;
+      if (sorted_axis && base + 4 <= n_e && !(r.c.flags & PV_ALWAYS)) {
+        if (r.c.flags & PV_NEVER) {
+          rng_on = true;
+          if (lane == 0) { ws.rg.n = 0.0; ws.rg.nend = -1.0; }
+        } else {
+          const double T0 = __ldg(tb), T1 = __ldg(tb + (n_e - 1));
+          const double x0 = (T0 - r.c.t0) * r.c.invP, x1 = (T1 - r.c.t0) * r.c.invP;
+          const double pad = 0x1p-49 * (fabs(x0) + fabs(x1) + 2.0);
+          const double n0 = ceil(x0 - r.c.ex_hi - pad), n1 = floor(x1 - r.c.ex_lo + pad);
+          if (n1 - n0 + 1.0 <= 0.0625 * (double)n_e + 2.0) {       // false for NaN/inf (they never reach here: the axis is finite)
+            rng_on = true;
+            if (lane == 0) {
+              ws.rg.n = n0; ws.rg.nend = n1;
+              ws.rg.T0 = T0;
+              ws.rg.idt = (T1 > T0) ? (double)(n_e - 1) / (T1 - T0) : 0.0;
+            }
+          }
+        }
+        __syncwarp();
+        rng_i = 0; rng_cnt = 0;
+      }
       phase = PH_STREAM;
       continue;
     }
@@ -975,30 +1105,125 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
   if (lane == 0) {
     const unsigned long long done = atomicAdd(A.sched + 1, 1ULL);
     if (done == (unsigned long long)nw - 1ULL) {   // every warp has taken its last ticket: nobody reads the slot any more
-      const int64_t nwords = 2 + (A.per_pv ? A.n_pv : 0);
+      const int64_t nwords = kSchedHead + (A.per_pv ? A.n_pv : 0);
       for (int64_t i = 0; i < nwords; ++i) A.sched[i] = 0ULL;
     }
   }
 }
 
-// Records of all parameter vectors, once per launch (single passband, few parameter vectors, many tiles each): a warp per
-// parameter vector runs the same setup the flux kernel would run per tile and stores the record to global memory; the
-// flux kernel then only copies it.  Raises the status flags (the flux kernel skips its own setup and with it the flags).
+// ---------------------------------------------------------------------------------------------------- prep kernel
+// Everything the flux kernel wants to find ready in its scheduler slot, in one small launch in front of it (the flux kernel
+// is its programmatic dependent: it starts launching at once and waits for this grid before it reads the slot).  Blocks
+// take one of four roles by index:
+//   records   a warp per parameter vector runs the per-tile setup once and stores the record (single passband, at most
+//             kPvCacheMax vectors with several tiles each: the flux kernel then only copies it per tile); raises the
+//             status flags that the flux kernel's own setup would have raised
+//   axis      is the shared time axis ascending and finite?  (range mode; kSlotUnsorted is set otherwise)
+//   order     row order of the tiles by counting sort on a 12-bit key: decreasing expected in-window fraction
+//             sqrt((1+k)² - b²)/(π a) + t_exp/P for the exact model (the estimate only orders tiles), k̂ for the table
+//   baseline  fused likelihood: partial sums of the all-out-of-transit chi2, fixed order; chi2[] zeroed
+struct PrepArgs {
+  PvRec* rec;
+  uint32_t* order;
+  int order_by_k;
+  int n_rec_blocks, n_axis_blocks, n_order_blocks, n_base_blocks;
+  double* base_part;
+};
+constexpr int kOrderBins = 4096;
+
 template <int MODE>
-__global__ void __launch_bounds__(kThreads) pv_cache_kernel(const __grid_constant__ FluxArgs A, PvRec* __restrict__ out) {
-  __shared__ WarpState s_ws[kWarpsPerBlock];
+__global__ void __launch_bounds__(kThreads) prep_kernel(const __grid_constant__ FluxArgs A, const __grid_constant__ PrepArgs Q) {
+  __shared__ WarpState s_ws[kWarpsPerBlock];          // records role; the other roles overlay their scratch on it
+  static_assert(sizeof(s_ws) >= kOrderBins * sizeof(int) + kThreads * sizeof(int), "order scratch must fit");
+  static_assert(sizeof(s_ws) >= kThreads * sizeof(double), "reduction scratch must fit");
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  WarpState& ws = s_ws[warp];
   asm volatile("griddepcontrol.launch_dependents;");   // the flux kernel may start launching: it waits before it reads
-  const int64_t pv = (int64_t)blockIdx.x * kWarpsPerBlock + warp;
-  if (pv >= A.n_pv) return;
-  tile_setup<MODE, true, double>(A, ws, 0, pv, 0, -1);
-  const double* src = reinterpret_cast<const double*>(&ws.pv[0]);
-  double* dst = reinterpret_cast<double*>(out + pv);
-  for (int i = lane; i < (int)(sizeof(PvRec) / sizeof(double)); i += 32) dst[i] = src[i];
-  // when this kernel was itself launched as a programmatic dependent (fused likelihood: of chi2_base_kernel), its
-  // completion must imply that kernel's: the flux kernel waits for this one only
-  asm volatile("griddepcontrol.wait;" ::: "memory");
+  int b = blockIdx.x;
+  if (b < Q.n_rec_blocks) {
+    const int64_t pv = (int64_t)b * kWarpsPerBlock + warp;
+    if (pv >= A.n_pv) return;
+    WarpState& ws = s_ws[warp];
+    tile_setup<MODE, true, double>(A, ws, 0, pv, 0, -1);
+    const double* src = reinterpret_cast<const double*>(&ws.pv[0]);
+    double* dst = reinterpret_cast<double*>(Q.rec + pv);
+    for (int i = lane; i < (int)(sizeof(PvRec) / sizeof(double)); i += 32) dst[i] = src[i];
+    return;
+  }
+  b -= Q.n_rec_blocks;
+  if (b < Q.n_axis_blocks) {
+    // adjacent pairs (j, j+1): NaN fails the comparison; the ends must be finite
+    bool bad = false;
+    const int64_t n = A.n_t;
+    for (int64_t j = (int64_t)b * kThreads + threadIdx.x; j + 1 < n; j += (int64_t)Q.n_axis_blocks * kThreads)
+      bad |= !(__ldg(A.times + j) <= __ldg(A.times + j + 1));
+    if (b == 0 && threadIdx.x == 0) bad |= !(fabs(__ldg(A.times)) < CUDART_INF) || !(fabs(__ldg(A.times + n - 1)) < CUDART_INF);
+    if (__any_sync(0xffffffffu, bad) && lane == 0) atomicOr(A.sched + 2, kSlotUnsorted);
+    return;
+  }
+  b -= Q.n_axis_blocks;
+  if (b < Q.n_order_blocks) {
+    int* hist = reinterpret_cast<int*>(s_ws);            // kOrderBins counters, then kThreads partial sums
+    int* part = hist + kOrderBins;
+    const int n = (int)A.n_pv;
+    for (int i = threadIdx.x; i < kOrderBins; i += kThreads) hist[i] = 0;
+    __syncthreads();
+    auto key_of = [&](int i) -> int {
+      const double* row = A.params + (int64_t)i * A.row_stride;
+      const double k = __ldg(row + 6 + 3 * A.pb_first);
+      float q;
+      if (Q.order_by_k) {
+        q = (float)((k - A.k_min) / (A.dk * (double)(A.n_k - 1)));              // position of k in the table's range
+      } else {
+        const double P = __ldg(row + 1), a = __ldg(row + 2), ci = cos(__ldg(row + 3));
+        const double bb = a * ci, c2 = (1.0 + k) * (1.0 + k) - bb * bb;
+        q = 1.0f - (float)(sqrt(fmax(c2, 0.0)) / (3.14159 * a) + ((A.n_ss > 1) ? fabs(A.t_exp / P) : 0.0));
+        if (!(q == q) || q > 1.0f || q < 0.0f) q = 0.0f;   // odd rows (bad parameters, a < 1+k): treat as heavy
+      }
+      if (!(q == q)) q = 0.0f;
+      return min(max((int)(q * (float)(kOrderBins - 1)), 0), kOrderBins - 1);
+    };
+    for (int i = threadIdx.x; i < n; i += kThreads) atomicAdd(&hist[key_of(i)], 1);
+    __syncthreads();
+    // exclusive scan of the histogram: each thread owns kOrderBins / kThreads consecutive bins
+    constexpr int kPer = kOrderBins / kThreads;
+    int sum = 0;
+    for (int j = 0; j < kPer; ++j) sum += hist[threadIdx.x * kPer + j];
+    part[threadIdx.x] = sum;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      int run = 0;
+      for (int t = 0; t < kThreads; ++t) { const int v = part[t]; part[t] = run; run += v; }
+    }
+    __syncthreads();
+    int run = part[threadIdx.x];
+    for (int j = 0; j < kPer; ++j) { const int v = hist[threadIdx.x * kPer + j]; hist[threadIdx.x * kPer + j] = run; run += v; }
+    __syncthreads();
+    for (int i = threadIdx.x; i < n; i += kThreads) Q.order[atomicAdd(&hist[key_of(i)], 1)] = (uint32_t)i;
+    return;
+  }
+  b -= Q.n_order_blocks;
+  {
+    // chi2 of the all-out-of-transit model, sum over (passband, exposure) of ((obs - 1) / sigma)²: block b reduces a
+    // contiguous range in a fixed order (strided per-thread sums, then a shared-memory tree) and writes one partial; the
+    // flux kernel adds the partials, again in a fixed order, to every parameter vector.
+    double* s_sum = reinterpret_cast<double*>(s_ws);
+    const int64_t n = (int64_t)A.n_pb * A.n_t;
+    const int64_t per = (n + Q.n_base_blocks - 1) / Q.n_base_blocks;
+    const int64_t lo = (int64_t)b * per, hi = min(lo + per, n);
+    double acc = 0.0;
+    for (int64_t i = lo + threadIdx.x; i < hi; i += kThreads) {
+      const double d = (__ldg(A.obs + i) - 1.0) * __ldg(A.isig + i);
+      acc = fma(d, d, acc);
+    }
+    s_sum[threadIdx.x] = acc;
+    __syncthreads();
+    for (int o = kThreads / 2; o > 0; o >>= 1) {
+      if ((int)threadIdx.x < o) s_sum[threadIdx.x] += s_sum[threadIdx.x + o];
+      __syncthreads();
+    }
+    if (threadIdx.x == 0) Q.base_part[b] = s_sum[0];
+    for (int64_t i = (int64_t)b * kThreads + threadIdx.x; i < A.n_pv; i += (int64_t)Q.n_base_blocks * kThreads) A.chi2[i] = 0.0;
+  }
 }
 
 }  // namespace pt

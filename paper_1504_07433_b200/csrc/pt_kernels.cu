@@ -6,6 +6,7 @@
 #include <stdint.h>
 
 #include <atomic>
+#include <mutex>
 
 #include "../../include/pt.h"
 #include "pt_flux.cuh"
@@ -14,31 +15,92 @@ namespace pt {
 
 static std::atomic<int64_t> g_launches{0};
 
-// Scheduler slots of the flux kernel (tile counters + finished-warp counter each).  A launch takes the next slot in a ring;
-// the kernel leaves its slot zeroed when it ends, so a slot is clean again long before the ring comes back to it (that
-// would need kSchedSlots launches in flight at once).  This is the only state the library keeps on the device.
-constexpr int kSchedSlots = 64;
-constexpr int kSchedWords = 1024;   // [0] global ticket, [1] finished warps, [2 + pv] per-parameter-vector tickets
-constexpr int kPvCacheMax = 512;    // parameter-vector records a slot can hold (pv_cache_kernel)
+// Scheduler slots of the flux kernel: tile counters, flag word, chi2 partials, row order and per-vector records, written by
+// prep_kernel / the flux kernel of ONE launch.  The kernel leaves the counters and flags of its slot zeroed when it ends.
+// Ordinary launches share the first kSchedRing slots round-robin per device; every launch records an event behind its
+// flux kernel, and a slot is given to a new launch only once that event has completed — if all of them are still in
+// flight, the new launch's stream is made to wait for the oldest one (cudaStreamWaitEvent: ordering on the device, no host
+// synchronisation), so two launches can never share a live slot whatever the number of streams and launches in flight.
+// A launch made while its stream is being captured into a CUDA graph gets one of the kSchedGraph slots behind the ring for
+// good (the graph replays it; CUDA orders replays of one executable graph behind one another) and makes no CUDA call
+// other than the kernel launches; when those slots are used up, capturing returns PT_ERR_CUDA.
+constexpr int kSchedRing = 16;
+constexpr int kSchedGraph = 8;
+constexpr int kSchedSlots = kSchedRing + kSchedGraph;
+constexpr int kSchedWords = 1024;   // [0] global ticket, [1] finished warps, [2] flags, [kSchedHead + pv] per-vector tickets;
+                                    // the last kBaseBlocks words hold the chi2 baseline partials
+constexpr int kPvCacheMax = 4096;   // parameter vectors whose records / row order a slot can hold (prep_kernel)
 struct SchedSlot {
   unsigned long long w[kSchedWords];
+  uint32_t order[kPvCacheMax];
   PvRec pv[kPvCacheMax];
 };
 __device__ SchedSlot g_sched[kSchedSlots];
-static std::atomic<uint64_t> g_sched_seq{0};
 
-static SchedSlot* sched_slot() {
-  static std::atomic<SchedSlot*> base[64];
+struct SlotHost {
+  cudaEvent_t ev = nullptr;
+  bool used = false;
+};
+struct DeviceSlots {
+  SchedSlot* base = nullptr;
+  SlotHost slot[kSchedRing];
+  int next = 0, n_graph = 0;
+};
+static std::mutex g_slot_mutex;
+static DeviceSlots g_dev_slots[64];
+
+struct SlotTicket {
+  SchedSlot* slot = nullptr;
+  int dev = -1, idx = -1;
+  bool capturing = false;
+};
+
+// Take a slot for a launch on `st` (see above).  Returns a null slot on a CUDA error or when the graph slots are used up.
+static SlotTicket slot_acquire(cudaStream_t st) {
+  SlotTicket t;
   int dev = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
-  SchedSlot* b = base[dev].load();
-  if (!b) {
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return t;
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) return t;
+  t.capturing = cs != cudaStreamCaptureStatusNone;
+  std::lock_guard<std::mutex> lock(g_slot_mutex);
+  DeviceSlots& D = g_dev_slots[dev];
+  if (!D.base) {
     void* p = nullptr;
-    if (cudaGetSymbolAddress(&p, g_sched) != cudaSuccess) return nullptr;
-    b = (SchedSlot*)p;
-    base[dev].store(b);
+    if (cudaGetSymbolAddress(&p, g_sched) != cudaSuccess) return t;
+    D.base = (SchedSlot*)p;
   }
-  return b + (g_sched_seq.fetch_add(1) % kSchedSlots);
+  t.dev = dev;
+  if (t.capturing) {
+    if (D.n_graph >= kSchedGraph) return t;
+    t.idx = kSchedRing + D.n_graph++;
+    t.slot = D.base + t.idx;
+    return t;
+  }
+  int pick = -1;
+  for (int k = 0; k < kSchedRing; ++k) {
+    const int i = (D.next + k) % kSchedRing;
+    SlotHost& h = D.slot[i];
+    if (!h.used || cudaEventQuery(h.ev) == cudaSuccess) { pick = i; break; }
+  }
+  (void)cudaGetLastError();            // cudaEventQuery's cudaErrorNotReady is not an error
+  if (pick < 0) {                      // every slot in flight: order this launch behind the oldest one
+    pick = D.next;
+    if (cudaStreamWaitEvent(st, D.slot[pick].ev, 0) != cudaSuccess) return t;
+  }
+  D.next = (pick + 1) % kSchedRing;
+  SlotHost& h = D.slot[pick];
+  if (!h.ev && cudaEventCreateWithFlags(&h.ev, cudaEventDisableTiming) != cudaSuccess) return t;
+  h.used = true;
+  t.slot = D.base + pick; t.idx = pick;
+  return t;
+}
+
+// Mark the end of the launch that holds the slot (after its last kernel has been enqueued on `st`).
+static void slot_release(const SlotTicket& t, cudaStream_t st) {
+  if (!t.slot || t.capturing) return;
+  std::lock_guard<std::mutex> lock(g_slot_mutex);
+  cudaEventRecord(g_dev_slots[t.dev].slot[t.idx].ev, st);
 }
 
 // S1-S2 alone: signed projected separation of every subsample.
@@ -98,31 +160,7 @@ __global__ void __launch_bounds__(kThreads) table_kernel(double k_min, double dk
   }
 }
 
-// Fused likelihood, step 1: chi2 of the all-out-of-transit model, sum over (passband, exposure) of ((obs - 1) / sigma)².
-// Block b reduces a contiguous range in a fixed order (strided per-thread sums, then a shared-memory tree) and writes one
-// partial; the flux kernel adds the partials, again in a fixed order, to every parameter vector.  Also zeroes chi2[].
-constexpr int kBaseBlocks = 128;
-__global__ void __launch_bounds__(kThreads) chi2_base_kernel(const double* __restrict__ obs, const double* __restrict__ isig,
-                                                             int64_t n, double* __restrict__ part, double* __restrict__ chi2,
-                                                             int64_t n_pv) {
-  __shared__ double s_sum[kThreads];
-  asm volatile("griddepcontrol.launch_dependents;");   // the record kernel does not read this kernel's output
-  const int64_t per = (n + gridDim.x - 1) / gridDim.x;
-  const int64_t lo = (int64_t)blockIdx.x * per, hi = min(lo + per, n);
-  double acc = 0.0;
-  for (int64_t i = lo + threadIdx.x; i < hi; i += kThreads) {
-    const double d = (__ldg(obs + i) - 1.0) * __ldg(isig + i);
-    acc = fma(d, d, acc);
-  }
-  s_sum[threadIdx.x] = acc;
-  __syncthreads();
-  for (int o = kThreads / 2; o > 0; o >>= 1) {
-    if (threadIdx.x < o) s_sum[threadIdx.x] += s_sum[threadIdx.x + o];
-    __syncthreads();
-  }
-  if (threadIdx.x == 0) part[blockIdx.x] = s_sum[0];
-  for (int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x; i < n_pv; i += (int64_t)gridDim.x * kThreads) chi2[i] = 0.0;
-}
+constexpr int kBaseBlocks = 128;   // chi2 baseline partials (prep_kernel), kept in the tail of the slot's words
 
 // FP64-pipe peak probe: 8 independent DFMA chains per thread.
 __global__ void __launch_bounds__(kThreads) dfma_probe_kernel(int iters, double* __restrict__ sink) {
@@ -145,6 +183,11 @@ static int check_common(const void* times, const void* params, const void* out, 
   return PT_OK;
 }
 
+static bool table_ok(const pt_table* tb) {
+  return tb && tb->d_data && tb->n_k >= 2 && tb->n_z >= 2 && (tb->n_fn == 3 || tb->n_fn == 4) && tb->dk > 0.0 && tb->dz > 0.0 &&
+         (tb->dtype == PT_F64 || tb->dtype == PT_F32);
+}
+
 // Number of SMs of the current device (the persistent grid is sized from it), cached per device.
 static int sm_count() {
   static std::atomic<int> cached[64];
@@ -164,6 +207,7 @@ static int sm_count() {
 //   mode 0  one global tile counter, rows in index order
 //   mode 1  one counter per parameter vector (a warp keeps its parameter vector: the setup is reused)
 //   mode 2  global counter, rows in order of decreasing expected work (LPT): heavy tiles first, the launch ends on light ones
+constexpr int64_t kLptRows = 512;   // rows up to which the longest-processing-time-first order is used
 struct Plan {
   int tile_len;
   int64_t tiles_per_pv;
@@ -172,6 +216,9 @@ struct Plan {
 };
 #ifndef PT_LPT_TILE
 #define PT_LPT_TILE 256
+#endif
+#ifndef PT_RANGE_MIN
+#define PT_RANGE_MIN 131072   // exposures (n_pv x n_t) from which the axis check + range mode pay for the extra launch
 #endif
 static Plan plan_tiles(int64_t n_pv, int64_t n_t, int n_sm) {
   Plan p{};
@@ -183,9 +230,9 @@ static Plan plan_tiles(int64_t n_pv, int64_t n_t, int n_sm) {
   if (tl < 256) tl = 256;
   if (tl > 16384) tl = 16384;
   int64_t tpp = (n_t + tl - 1) / tl;
-  const bool few = (n_pv <= kSchedWords - 2 - kBaseBlocks && tpp >= 2);   // the slot's tail holds the chi2 partials
+  const bool few = (n_pv <= kSchedWords - kSchedHead - kBaseBlocks && tpp >= 2);   // the slot's tail holds the chi2 partials
   p.mode = few ? 1 : 0;
-  if (few && n_pv <= kLptMax && n_pv * tpp >= 2 * warps) {   // worth ranking the rows only with several tiles per warp
+  if (few && n_pv <= kLptRows && n_pv * tpp >= 2 * warps) {   // worth ranking the rows only with several tiles per warp
     p.mode = 2;
     if (tl < PT_LPT_TILE) { tl = PT_LPT_TILE; tpp = (n_t + tl - 1) / tl; }
   }
@@ -220,16 +267,14 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
     A.flux_pv_stride = (int64_t)n_pb_row * n_t; A.flux_off = (int64_t)pb_view * n_t;
   }
   if (mode == 1) {
-    if (!tb || !tb->d_data || tb->n_k < 2 || tb->n_z < 2 || (tb->n_fn != 3 && tb->n_fn != 4) || !(tb->dk > 0.0) ||
-        !(tb->dz > 0.0) || (tb->dtype != PT_F64 && tb->dtype != PT_F32))
-      return PT_ERR_TABLE;
+    if (!table_ok(tb)) return PT_ERR_TABLE;
     A.tb = tb->d_data; A.tb_dtype = tb->dtype; A.n_k = tb->n_k; A.n_z = tb->n_z; A.n_fn = tb->n_fn;
-    A.k_min = tb->k_min; A.dk = tb->dk; A.dz = tb->dz;
+    A.k_min = tb->k_min; A.dk = tb->dk; A.dz = tb->dz; A.inv_dz = 1.0 / tb->dz;
   }
   const pt::Plan plan = plan_tiles(n_pv, n_t, sm_count());
   if (plan.tile_len == 0) return PT_ERR_SIZE;
   A.tile_len = plan.tile_len; A.tiles_per_pv = (int)plan.tiles_per_pv; A.n_tiles = n_pv * plan.tiles_per_pv;
-  A.per_pv = plan.mode == 1; A.lpt = plan.mode == 2;
+  A.per_pv = plan.mode == 1;
   int lg = 0;
   while (((int64_t)1 << lg) < (int64_t)n_ss) ++lg;
   A.fx_bits = 61 - lg;
@@ -237,50 +282,59 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   A.fx_inv = 1.0 / (A.fx_scale * (double)n_ss);
   A.inv_nss = 1.0 / (double)n_ss;
   const dim3 grid((unsigned)plan.blocks);
-  SchedSlot* slot = sched_slot();
+  if (dtype == kDtypeChi2) {
+    A.obs = like->obs; A.isig = like->isig; A.chi2 = (double*)d_flux; A.flux = nullptr;
+  }
+  const SlotTicket ticket = slot_acquire(st);
+  SchedSlot* slot = ticket.slot;
   if (!slot) return PT_ERR_CUDA;
   A.sched = slot->w;
-  // single passband, few parameter vectors, many tiles each: the per-vector records are computed once, by a small kernel
-  // in front of the flux kernel (the setup is 15 % of the flux kernel's instructions on configs[1] when done per tile)
-  if (n_pb == 1 && pb_view < 0 && n_pv <= kPvCacheMax && A.n_tiles >= 8 * n_pv) {
-    const unsigned nb = (unsigned)((n_pv + kWarpsPerBlock - 1) / kWarpsPerBlock);
-    // fused likelihood: the record kernel overlaps chi2_base_kernel (it waits for it only before it exits, so that the
-    // flux kernel, which waits for the record kernel, also sees the baseline)
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
-    cudaLaunchConfig_t c2{};
-    c2.gridDim = dim3(nb); c2.blockDim = dim3(kThreads); c2.dynamicSmemBytes = 0; c2.stream = st;
-    c2.attrs = at; c2.numAttrs = (dtype == kDtypeChi2) ? 1 : 0;
-    if (mode == 0) cudaLaunchKernelEx(&c2, pv_cache_kernel<0>, A, slot->pv);
-    else cudaLaunchKernelEx(&c2, pv_cache_kernel<1>, A, slot->pv);
-    A.pvcache = slot->pv;
-    g_launches.fetch_add(1);
-  }
+  // What prep_kernel is asked to leave in the slot (pt_flux.cuh):
+  //   records  single passband, at most kPvCacheMax parameter vectors, many tiles each (the per-tile setup is 15 % of the
+  //            flux kernel's instructions on configs[1] when done per tile)
+  //   axis     one shared time axis of a problem large enough for the extra launch to pay: is it ascending?
+  //   order    global tile counter: heaviest rows first (mode 2), or rows by k̂ for the interpolated model
+  //   baseline fused likelihood
+  const bool want_rec = n_pb == 1 && pb_view < 0 && n_pv <= kPvCacheMax && A.n_tiles >= 8 * n_pv;
+  const bool want_axis = t_stride_pv == 0 && n_t >= 512 && (double)n_pv * (double)n_t >= (double)PT_RANGE_MIN;
+  const bool want_order = n_pv <= kPvCacheMax && n_pv >= 2 &&
+                          (plan.mode == 2 || (mode == 1 && plan.mode == 0 && A.n_tiles >= 4 * (int64_t)grid.x * kWarpsPerBlock));
+  PrepArgs Q{};
+  if (want_rec) { Q.rec = slot->pv; Q.n_rec_blocks = (int)((n_pv + kWarpsPerBlock - 1) / kWarpsPerBlock); }
+  if (want_axis) { int nb = (int)((n_t + 8 * kThreads - 1) / (8 * kThreads)); Q.n_axis_blocks = nb > 64 ? 64 : nb; }
+  if (want_order) { Q.order = slot->order; Q.order_by_k = (plan.mode == 0) ? 1 : 0; Q.n_order_blocks = 1; }
   if (dtype == kDtypeChi2) {
-    // step 1 of the fused likelihood: out-of-transit baseline into the tail of the scheduler slot, chi2[] zeroed
-    double* part = reinterpret_cast<double*>(A.sched + kSchedWords - kBaseBlocks);
+    // out-of-transit baseline into the tail of the slot's words, chi2[] zeroed
     const int64_t n_obs = (int64_t)n_pb * n_t;
     int nb = (int)((n_obs + 4095) / 4096);
-    if (nb > kBaseBlocks) nb = kBaseBlocks;
-    if (nb < 1) nb = 1;
-    chi2_base_kernel<<<nb, kThreads, 0, st>>>(like->obs, like->isig, n_obs, part, (double*)d_flux, n_pv);
+    Q.n_base_blocks = nb > kBaseBlocks ? kBaseBlocks : (nb < 1 ? 1 : nb);
+    Q.base_part = reinterpret_cast<double*>(A.sched + kSchedWords - kBaseBlocks);
+    A.base_part = Q.base_part; A.n_base_part = Q.n_base_blocks;
+  }
+  const int n_prep = Q.n_rec_blocks + Q.n_axis_blocks + Q.n_order_blocks + Q.n_base_blocks;
+  if (n_prep > 0) {
+    // an ordinary launch: ordered behind whatever the caller enqueued before (the kernel that wrote d_params, the fill that
+    // zeroed d_status), so it and its dependent below see the caller's data
+    if (mode == 0) prep_kernel<0><<<n_prep, kThreads, 0, st>>>(A, Q);
+    else prep_kernel<1><<<n_prep, kThreads, 0, st>>>(A, Q);
     g_launches.fetch_add(1);
-    A.obs = like->obs; A.isig = like->isig; A.chi2 = (double*)d_flux; A.base_part = part; A.n_base_part = nb;
-    A.flux = nullptr;
+    A.prep = 1;
+    A.pvcache = want_rec ? slot->pv : nullptr;
+    A.order = want_order ? slot->order : nullptr;
+    A.range = want_axis ? 1 : 0;
   }
   // 16-byte loads/stores need even row lengths/strides and 16-byte aligned bases
   const bool v2 = (n_t % 2 == 0) && (t_stride_pv % 2 == 0) && (reinterpret_cast<uintptr_t>(d_times) % 16 == 0) &&
                   (dtype == kDtypeChi2 || reinterpret_cast<uintptr_t>(d_flux) % 16 == 0);
   const bool p1 = (n_pb == 1), s1 = (n_ss == 1);
-  // with the record cache the flux kernel is launched as a programmatic dependent of pv_cache_kernel: its launch and its
-  // prologue (row ranking) overlap that kernel, and it waits (griddepcontrol.wait) before it reads the first record
+  // behind prep_kernel the flux kernel is a programmatic dependent launch: its launch latency overlaps that kernel, and it
+  // waits (griddepcontrol.wait) before it reads the slot
   cudaLaunchAttribute pdl_attr[1];
   pdl_attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   pdl_attr[0].val.programmaticStreamSerializationAllowed = 1;
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = grid; cfg.blockDim = dim3(kThreads); cfg.dynamicSmemBytes = 0; cfg.stream = st;
-  cfg.attrs = pdl_attr; cfg.numAttrs = A.pvcache ? 1 : 0;
+  cfg.attrs = pdl_attr; cfg.numAttrs = A.prep ? 1 : 0;
 #define PT_LAUNCH(M, VV, P, S, T) cudaLaunchKernelEx(&cfg, flux_kernel<M, VV, P, S, T>, A)
 #define PT_LAUNCH_S(M, VV, P, T)                             \
   do {                                                       \
@@ -303,7 +357,9 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
 #undef PT_LAUNCH_S
 #undef PT_LAUNCH
   g_launches.fetch_add(1);
-  return cudaGetLastError() == cudaSuccess ? PT_OK : PT_ERR_CUDA;
+  const cudaError_t err = cudaGetLastError();
+  slot_release(ticket, st);
+  return err == cudaSuccess ? PT_OK : PT_ERR_CUDA;
 }
 
 }  // namespace pt
@@ -344,7 +400,7 @@ int pt_orbit_z(const double* d_times, int64_t n_t, int64_t t_stride_pv, const do
   if (rc) return rc;
   const int64_t n = n_t * n_ss;
   int64_t bpp = (n + (int64_t)kThreads * 8 - 1) / ((int64_t)kThreads * 8);
-  const int64_t cap = (148 * 16 + n_pv - 1) / n_pv;
+  const int64_t cap = ((int64_t)sm_count() * 16 + n_pv - 1) / n_pv;
   if (bpp > cap) bpp = cap;
   if (bpp < 1) bpp = 1;
   if (n_pv * bpp > 0x7fffffff) return PT_ERR_SIZE;
@@ -375,16 +431,25 @@ int pt_ma_quad_exact_pbk(const double* d_times, int64_t n_t, int64_t t_stride_pv
   return rc;
 }
 
+int pt_table_spacing(double k_min, double k_max, int32_t n_k, double z_max, int32_t n_z, double* h_dk, double* h_dz) {
+  if (!h_dk || !h_dz) return PT_ERR_NULL;
+  if (n_k < 2 || n_z < 2 || !(k_max > k_min) || !(k_min >= 0.0) || !(z_max > 0.0)) return PT_ERR_SIZE;
+  *h_dk = (k_max - k_min) / (double)(n_k - 1);
+  *h_dz = z_max / (double)(n_z - 1);
+  return PT_OK;
+}
+
 int pt_ma_table_build(double k_min, double k_max, int32_t n_k, double z_max, int32_t n_z, int32_t dtype, int32_t n_fn,
                       void* d_table, void* stream) {
   if (!d_table) return PT_ERR_NULL;
   if (n_k < 2 || n_z < 2 || (n_fn != 3 && n_fn != 4) || !(k_max > k_min) || !(k_min >= 0.0) || !(z_max > 0.0))
     return PT_ERR_SIZE;
   if (dtype != PT_F64 && dtype != PT_F32) return PT_ERR_DTYPE;
-  const double dk = (k_max - k_min) / (double)(n_k - 1), dz = z_max / (double)(n_z - 1);
+  double dk, dz;
+  pt_table_spacing(k_min, k_max, n_k, z_max, n_z, &dk, &dz);
   const int64_t n = (int64_t)n_k * n_z;
   int64_t blocks = (n + kThreads - 1) / kThreads;
-  if (blocks > 148 * 64) blocks = 148 * 64;
+  if (blocks > (int64_t)sm_count() * 64) blocks = (int64_t)sm_count() * 64;
   if (dtype == PT_F64)
     table_kernel<double><<<(unsigned)blocks, kThreads, 0, (cudaStream_t)stream>>>(k_min, dk, n_k, dz, n_z, n_fn, (double*)d_table);
   else
@@ -410,47 +475,60 @@ int pt_ma_quad_chi2(const pt_table* table, const double* d_times, int64_t n_t, c
 }
 
 // ---- host-buffer forms: H2D, kernels, D2H on an internal stream, then wait.
+// Scratch of the calling thread on one device: a stream and four grow-only device buffers (times, parameters, flux, status),
+// kept between calls so that a steady-state call allocates nothing; freed when the thread ends.
+struct HostScratch {
+  cudaStream_t st = nullptr;
+  void* buf[4] = {nullptr, nullptr, nullptr, nullptr};
+  size_t cap[4] = {0, 0, 0, 0};
+  ~HostScratch() {
+    for (void* b : buf) if (b) cudaFree(b);
+    if (st) cudaStreamDestroy(st);
+  }
+  bool reserve(int i, size_t bytes) {
+    if (bytes <= cap[i]) return true;
+    if (buf[i]) { cudaFree(buf[i]); buf[i] = nullptr; cap[i] = 0; }
+    const size_t want = bytes + bytes / 4;
+    if (cudaMalloc(&buf[i], want) != cudaSuccess) return false;
+    cap[i] = want;
+    return true;
+  }
+};
+
 static int run_host(int mode, const pt_table* tb, const double* h_times, int64_t n_t, int64_t t_stride_pv,
                     const double* h_params, int64_t n_pv, int n_pb, int n_ss, double t_exp, int dtype, void* h_flux,
                     int32_t* h_status) {
+  // every argument error is reported before anything is allocated or enqueued
   int rc = check_common(h_times, h_params, h_flux, n_t, t_stride_pv, n_pv, n_pb, n_ss);
   if (rc) return rc;
   if (dtype != PT_F64 && dtype != PT_F32) return PT_ERR_DTYPE;
-  static thread_local cudaStream_t st = nullptr;
-  if (!st) {
-    if (cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) != cudaSuccess) return PT_ERR_CUDA;
-    // keep the stream-ordered scratch in the pool between calls (the default hands it back at every synchronisation)
-    int dev = 0;
-    cudaMemPool_t pool;
-    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-      uint64_t keep = UINT64_MAX;
-      cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-    }
-  }
+  if (mode == 1 && !table_ok(tb)) return PT_ERR_TABLE;
+  if (plan_tiles(n_pv, n_t, sm_count()).tile_len == 0) return PT_ERR_SIZE;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return PT_ERR_CUDA;
+  static thread_local HostScratch scratch[64];      // one per device: the stream belongs to the device it was created on
+  HostScratch& S = scratch[dev];
+  if (!S.st && cudaStreamCreateWithFlags(&S.st, cudaStreamNonBlocking) != cudaSuccess) return PT_ERR_CUDA;
   const size_t nb_t = sizeof(double) * (size_t)(t_stride_pv == 0 ? n_t : (n_pv - 1) * t_stride_pv + n_t);
   const size_t nb_p = sizeof(double) * (size_t)n_pv * (6 + 3 * (size_t)n_pb);
   const size_t nb_f = (dtype == PT_F64 ? 8 : 4) * (size_t)n_pv * n_pb * n_t;
-  double *d_t = nullptr, *d_p = nullptr;
-  void* d_f = nullptr;
-  int32_t* d_s = nullptr;
-  bool ok = cudaMallocAsync(&d_t, nb_t, st) == cudaSuccess && cudaMallocAsync(&d_p, nb_p, st) == cudaSuccess &&
-            cudaMallocAsync(&d_f, nb_f, st) == cudaSuccess && cudaMallocAsync(&d_s, 8, st) == cudaSuccess;
-  if (ok) {
-    cudaMemcpyAsync(d_t, h_times, nb_t, cudaMemcpyHostToDevice, st);
-    cudaMemcpyAsync(d_p, h_params, nb_p, cudaMemcpyHostToDevice, st);
-    cudaMemsetAsync(d_s, 0, 8, st);
-    rc = launch_flux(mode, tb, d_t, n_t, t_stride_pv, d_p, n_pv, n_pb, n_ss, t_exp, dtype, d_f, d_s, st);
-    if (rc == PT_OK) {
-      cudaMemcpyAsync(h_flux, d_f, nb_f, cudaMemcpyDeviceToHost, st);
-      if (h_status) cudaMemcpyAsync(h_status, d_s, 8, cudaMemcpyDeviceToHost, st);
-    }
-  } else {
-    rc = PT_ERR_CUDA;
+  if (!(S.reserve(0, nb_t) && S.reserve(1, nb_p) && S.reserve(2, nb_f) && S.reserve(3, 8))) {
+    (void)cudaGetLastError();
+    return PT_ERR_CUDA;
   }
-  if (d_t) cudaFreeAsync(d_t, st);
-  if (d_p) cudaFreeAsync(d_p, st);
-  if (d_f) cudaFreeAsync(d_f, st);
-  if (d_s) cudaFreeAsync(d_s, st);
+  cudaStream_t st = S.st;
+  double* d_t = (double*)S.buf[0];
+  double* d_p = (double*)S.buf[1];
+  void* d_f = S.buf[2];
+  int32_t* d_s = (int32_t*)S.buf[3];
+  cudaMemcpyAsync(d_t, h_times, nb_t, cudaMemcpyHostToDevice, st);
+  cudaMemcpyAsync(d_p, h_params, nb_p, cudaMemcpyHostToDevice, st);
+  cudaMemsetAsync(d_s, 0, 8, st);
+  rc = launch_flux(mode, tb, d_t, n_t, t_stride_pv, d_p, n_pv, n_pb, n_ss, t_exp, dtype, d_f, d_s, st);
+  if (rc == PT_OK) {
+    cudaMemcpyAsync(h_flux, d_f, nb_f, cudaMemcpyDeviceToHost, st);
+    if (h_status) cudaMemcpyAsync(h_status, d_s, 8, cudaMemcpyDeviceToHost, st);
+  }
   if (cudaStreamSynchronize(st) != cudaSuccess && rc == PT_OK) rc = PT_ERR_CUDA;
   return rc;
 }
