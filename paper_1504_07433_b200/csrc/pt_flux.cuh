@@ -54,6 +54,11 @@ constexpr int kMaxTileLen = 32768;
 constexpr int kRemBias = 1 << 24;
 constexpr int kSchedHead = 8;   // words of a scheduler slot in front of the per-parameter-vector tickets
 constexpr unsigned long long kSlotUnsorted = 1ULL;   // flag word: the shared time axis is not ascending / not finite
+// words of a scheduler slot: [0] tile / work ticket, [1] warps (blocks) that have finished, [2] flags, [3] prep blocks that
+// have finished (fused likelihood in front of the epoch kernel)
+enum { kW_Ticket = 0, kW_Done = 1, kW_Flags = 2, kW_PrepDone = 3 };
+constexpr uint32_t kUnitChunks = 0x80000000u;        // ucnt flag: units are chunks of kChunkLen exposures, not transit epochs
+constexpr int kChunkLen = 256;
 // -DPT_DEBUG_CHECKS: capacity invariants of the per-warp queues are checked and a violation traps (the test suite is run
 // once against such a build; compute-sanitizer is not available on the GPU pool).
 #ifdef PT_DEBUG_CHECKS
@@ -100,10 +105,16 @@ struct FluxArgs {
   const PvRec* pvcache;        // single passband, few parameter vectors: records precomputed by prep_kernel (else NULL)
   const uint32_t* order;       // global mode: row order of the tiles written by prep_kernel (heaviest rows first / rows sorted
                                // by k̂ for the table), or NULL = index order
+  int epoch;                   // 1: this launch runs behind the epoch kernel and only acts if the axis turned out unsorted
   int per_pv;                  // 1: warps stay on one parameter vector and take its tiles from its own counter (n_pv small)
   int prep;                    // 1: launched as a programmatic dependent of prep_kernel: wait for it before reading the slot
   int range;                   // 1: one shared time axis; if prep_kernel found it ascending and finite, out-of-window
                                // stretches are found by search and written as pure fills (no per-exposure window test)
+  // epoch kernel (pt_epoch.cuh): units of evaluation work per parameter vector, written by prep_kernel
+  const double* un0;           // [n_pv] first transit epoch on the axis (units in epoch mode)
+  const uint32_t* ucnt;        // [n_pv] number of units; kUnitChunks set: the row is cut into chunks of kChunkLen exposures
+  int unit_chunks;             // work units per row: unit (row, c) owns the epochs [c cnt/C, (c+1) cnt/C) and the gaps in front of them
+  int base_added;              // fused likelihood: prep_kernel already left the baseline in chi2[]
   // supersample accumulation (fixed point)
   int fx_bits;             // 61 - ceil(log2 n_ss): a sum of n_ss values below 2^eb fits an int64 at scale 2^(fx_bits-eb)
   double fx_scale;         // 2^fx_bits (basis values are <= 1)
@@ -833,7 +844,8 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
   // in flight then share a few k-rows of the table, which stay in L1/L2 while gigabytes of flux stream past).
   // The slot (order, records, flags) is written by prep_kernel, whose programmatic dependent this grid is.
   if (A.prep) asm volatile("griddepcontrol.wait;" ::: "memory");
-  const bool sorted_axis = A.range && !(*((volatile const unsigned long long*)(A.sched + 2)) & kSlotUnsorted);
+  const bool sorted_axis = A.range && !(*((volatile const unsigned long long*)(A.sched + kW_Flags)) & kSlotUnsorted);
+  if (A.epoch && sorted_axis) return;   // the epoch kernel in front of this one did the whole launch (and cleaned the slot)
   const int tpp = A.tiles_per_pv;
   int64_t pv_cur = 0, last_pv = -1;
   int chunk_cur = 0, last_ring = -1;
@@ -1055,14 +1067,14 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
       keep = EPW;
       if (r.c.flags & PV_BAD) {
         if constexpr (kIsChi2<OutT>) {
-          if (chunk_cur == 0 && lane == 0) atomicAdd(A.chi2 + pv_cur, nan64());
+          if (chunk_cur == 0 && lane == 0 && !A.base_added) atomicAdd(A.chi2 + pv_cur, nan64());
         } else {
           for (int j = 0; j < n_pb; ++j)
             for (uint32_t e = lane; e < n_e; e += 32) ob[(int64_t)j * A.n_t + e] = (OutT)nan64();
         }
         base = n_e;       // nothing to stream
         keep = 1;
-      } else if (kIsChi2<OutT> && chunk_cur == 0) {
+      } else if (kIsChi2<OutT> && chunk_cur == 0 && !A.base_added) {
         // chi2 of this parameter vector starts from the all-out-of-transit value: partial sums in fixed order
         double b = 0.0;
         for (int i = lane; i < A.n_base_part; i += 32) b += A.base_part[i];
@@ -1128,12 +1140,36 @@ struct PrepArgs {
   int order_by_k;
   int n_rec_blocks, n_axis_blocks, n_order_blocks, n_base_blocks;
   double* base_part;
+  // units of the epoch kernel (pt_epoch.cuh): per-row first epoch and unit count (records role)
+  double* un0;
+  uint32_t* ucnt;
+  int want_units;
+  int n_blocks;              // blocks of this launch
 };
 constexpr int kOrderBins = 4096;
+
+// Units of evaluation work of one parameter vector on the shared ascending axis [T_first, T_last] (epoch kernel): the
+// transit epochs n0 .. n0 + cnt - 1 whose window [t0 + (n + ex_lo) P, t0 + (n + ex_hi) P] can hold an exposure, or — a row
+// that is always in the window, or whose windows are so dense that looking for them costs more than evaluating every
+// exposure — chunks of kChunkLen exposures (kUnitChunks).  Rows that never transit or are bad have no units.
+__device__ __forceinline__ void pv_units(const PvConst& c, double T_first, double T_last, int64_t n_t, double* n0, uint32_t* cnt) {
+  *n0 = 0.0; *cnt = 0u;
+  if (c.flags & (PV_BAD | PV_NEVER)) return;
+  const uint32_t chunks = kUnitChunks | (uint32_t)((n_t + kChunkLen - 1) / kChunkLen);
+  if (c.flags & PV_ALWAYS) { *cnt = chunks; return; }
+  const double x0 = (T_first - c.t0) * c.invP, x1 = (T_last - c.t0) * c.invP;
+  const double pad = 0x1p-49 * (fabs(x0) + fabs(x1) + 2.0);
+  const double a = ceil(x0 - c.ex_hi - pad), b = floor(x1 - c.ex_lo + pad);
+  const double m = b - a + 1.0;
+  if (!(m >= 1.0)) return;                                  // no epoch on the axis (or a non-finite axis: never used then)
+  if (m > 0.125 * (double)n_t + 2.0 || m > 1.0e9) { *cnt = chunks; return; }
+  *n0 = a; *cnt = (uint32_t)m;
+}
 
 template <int MODE>
 __global__ void __launch_bounds__(kThreads) prep_kernel(const __grid_constant__ FluxArgs A, const __grid_constant__ PrepArgs Q) {
   __shared__ WarpState s_ws[kWarpsPerBlock];          // records role; the other roles overlay their scratch on it
+  __shared__ int s_last;
   static_assert(sizeof(s_ws) >= kOrderBins * sizeof(int) + kThreads * sizeof(int), "order scratch must fit");
   static_assert(sizeof(s_ws) >= kThreads * sizeof(double), "reduction scratch must fit");
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -1141,27 +1177,27 @@ __global__ void __launch_bounds__(kThreads) prep_kernel(const __grid_constant__ 
   int b = blockIdx.x;
   if (b < Q.n_rec_blocks) {
     const int64_t pv = (int64_t)b * kWarpsPerBlock + warp;
-    if (pv >= A.n_pv) return;
-    WarpState& ws = s_ws[warp];
-    tile_setup<MODE, true, double>(A, ws, 0, pv, 0, -1);
-    const double* src = reinterpret_cast<const double*>(&ws.pv[0]);
-    double* dst = reinterpret_cast<double*>(Q.rec + pv);
-    for (int i = lane; i < (int)(sizeof(PvRec) / sizeof(double)); i += 32) dst[i] = src[i];
-    return;
-  }
-  b -= Q.n_rec_blocks;
-  if (b < Q.n_axis_blocks) {
+    if (pv < A.n_pv) {
+      WarpState& ws = s_ws[warp];
+      tile_setup<MODE, true, double>(A, ws, 0, pv, 0, -1);
+      const double* src = reinterpret_cast<const double*>(&ws.pv[0]);
+      double* dst = reinterpret_cast<double*>(Q.rec + pv);
+      for (int i = lane; i < (int)(sizeof(PvRec) / sizeof(double)); i += 32) dst[i] = src[i];
+      if (Q.want_units && lane == 0) {
+        double n0; uint32_t cnt;
+        pv_units(ws.pv[0].c, __ldg(A.times), __ldg(A.times + A.n_t - 1), A.n_t, &n0, &cnt);
+        Q.un0[pv] = n0; Q.ucnt[pv] = cnt;
+      }
+    }
+  } else if ((b -= Q.n_rec_blocks) < Q.n_axis_blocks) {
     // adjacent pairs (j, j+1): NaN fails the comparison; the ends must be finite
     bool bad = false;
     const int64_t n = A.n_t;
     for (int64_t j = (int64_t)b * kThreads + threadIdx.x; j + 1 < n; j += (int64_t)Q.n_axis_blocks * kThreads)
       bad |= !(__ldg(A.times + j) <= __ldg(A.times + j + 1));
     if (b == 0 && threadIdx.x == 0) bad |= !(fabs(__ldg(A.times)) < CUDART_INF) || !(fabs(__ldg(A.times + n - 1)) < CUDART_INF);
-    if (__any_sync(0xffffffffu, bad) && lane == 0) atomicOr(A.sched + 2, kSlotUnsorted);
-    return;
-  }
-  b -= Q.n_axis_blocks;
-  if (b < Q.n_order_blocks) {
+    if (__any_sync(0xffffffffu, bad) && lane == 0) atomicOr(A.sched + kW_Flags, kSlotUnsorted);
+  } else if ((b -= Q.n_axis_blocks) < Q.n_order_blocks) {
     int* hist = reinterpret_cast<int*>(s_ws);            // kOrderBins counters, then kThreads partial sums
     int* part = hist + kOrderBins;
     const int n = (int)A.n_pv;
@@ -1199,10 +1235,8 @@ __global__ void __launch_bounds__(kThreads) prep_kernel(const __grid_constant__ 
     for (int j = 0; j < kPer; ++j) { const int v = hist[threadIdx.x * kPer + j]; hist[threadIdx.x * kPer + j] = run; run += v; }
     __syncthreads();
     for (int i = threadIdx.x; i < n; i += kThreads) Q.order[atomicAdd(&hist[key_of(i)], 1)] = (uint32_t)i;
-    return;
-  }
-  b -= Q.n_order_blocks;
-  {
+  } else {
+    b -= Q.n_order_blocks;
     // chi2 of the all-out-of-transit model, sum over (passband, exposure) of ((obs - 1) / sigma)²: block b reduces a
     // contiguous range in a fixed order (strided per-thread sums, then a shared-memory tree) and writes one partial; the
     // flux kernel adds the partials, again in a fixed order, to every parameter vector.
@@ -1222,8 +1256,27 @@ __global__ void __launch_bounds__(kThreads) prep_kernel(const __grid_constant__ 
       __syncthreads();
     }
     if (threadIdx.x == 0) Q.base_part[b] = s_sum[0];
-    for (int64_t i = (int64_t)b * kThreads + threadIdx.x; i < A.n_pv; i += (int64_t)Q.n_base_blocks * kThreads) A.chi2[i] = 0.0;
+    if (!Q.want_units)
+      for (int64_t i = (int64_t)b * kThreads + threadIdx.x; i < A.n_pv; i += (int64_t)Q.n_base_blocks * kThreads) A.chi2[i] = 0.0;
   }
+  if (!Q.want_units || Q.n_base_blocks == 0) return;
+  // ---- fused likelihood in front of the epoch kernel: the last block to get here leaves the out-of-transit baseline (the
+  // partials in a fixed order) in chi2[]; bad rows are NaN
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    s_last = (atomicAdd(A.sched + kW_PrepDone, 1ULL) == (unsigned long long)(Q.n_blocks - 1)) ? 1 : 0;
+  }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  double B = 0.0;
+  for (int i = 0; i < Q.n_base_blocks; ++i) B += ((volatile double*)Q.base_part)[i];
+  for (int pv = threadIdx.x; pv < (int)A.n_pv; pv += kThreads) {
+    const int fl = ((volatile int*)&Q.rec[pv].c.flags)[0];
+    A.chi2[pv] = (fl & PV_BAD) ? nan64() : B;
+  }
+  if (threadIdx.x == 0) A.sched[kW_PrepDone] = 0ULL;
 }
 
 }  // namespace pt

@@ -10,6 +10,7 @@
 
 #include "../../include/pt.h"
 #include "pt_flux.cuh"
+#include "pt_epoch.cuh"
 
 namespace pt {
 
@@ -34,6 +35,9 @@ struct SchedSlot {
   unsigned long long w[kSchedWords];
   uint32_t order[kPvCacheMax];
   PvRec pv[kPvCacheMax];
+  // epoch kernel (pt_epoch.cuh): first epoch and unit count per row, prefix of the batch counts in row order
+  double un0[kPvCacheMax];
+  uint32_t ucnt[kPvCacheMax];
 };
 __device__ SchedSlot g_sched[kSchedSlots];
 
@@ -297,12 +301,16 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   //   baseline fused likelihood
   const bool want_rec = n_pb == 1 && pb_view < 0 && n_pv <= kPvCacheMax && A.n_tiles >= 8 * n_pv;
   const bool want_axis = t_stride_pv == 0 && n_t >= 512 && (double)n_pv * (double)n_t >= (double)PT_RANGE_MIN;
+  // epoch kernel: one passband on one shared axis that prep_kernel checks; it does the whole launch if the axis is ascending,
+  // else the general kernel launched behind it does
+  const bool want_epoch = want_axis && n_pb == 1 && pb_view < 0 && n_pv <= kPvCacheMax && n_t < 0x7fffff00LL &&
+                          (mode == 0 || (size_t)tb->n_z * sizeof(double) <= 110000);
   const bool want_order = n_pv <= kPvCacheMax && n_pv >= 2 &&
-                          (plan.mode == 2 || (mode == 1 && plan.mode == 0 && A.n_tiles >= 4 * (int64_t)grid.x * kWarpsPerBlock));
+                          (want_epoch || plan.mode == 2 || (mode == 1 && plan.mode == 0 && A.n_tiles >= 4 * (int64_t)grid.x * kWarpsPerBlock));
   PrepArgs Q{};
-  if (want_rec) { Q.rec = slot->pv; Q.n_rec_blocks = (int)((n_pv + kWarpsPerBlock - 1) / kWarpsPerBlock); }
+  if (want_rec || want_epoch) { Q.rec = slot->pv; Q.n_rec_blocks = (int)((n_pv + kWarpsPerBlock - 1) / kWarpsPerBlock); }
   if (want_axis) { int nb = (int)((n_t + 8 * kThreads - 1) / (8 * kThreads)); Q.n_axis_blocks = nb > 64 ? 64 : nb; }
-  if (want_order) { Q.order = slot->order; Q.order_by_k = (plan.mode == 0) ? 1 : 0; Q.n_order_blocks = 1; }
+  if (want_order) { Q.order = slot->order; Q.order_by_k = (want_epoch ? mode == 1 : plan.mode == 0) ? 1 : 0; Q.n_order_blocks = 1; }
   if (dtype == kDtypeChi2) {
     // out-of-transit baseline into the tail of the slot's words, chi2[] zeroed
     const int64_t n_obs = (int64_t)n_pb * n_t;
@@ -312,6 +320,18 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
     A.base_part = Q.base_part; A.n_base_part = Q.n_base_blocks;
   }
   const int n_prep = Q.n_rec_blocks + Q.n_axis_blocks + Q.n_order_blocks + Q.n_base_blocks;
+  // epoch kernel: interpolated model = blocks of 16 warps that stage the table (n_z doubles of shared memory, two per SM);
+  // exact model = single-warp blocks, 24 per SM.  About four units per block so that the ticket counter balances the load.
+  const int e_nt = (mode == 1) ? 512 : 32;
+  const int64_t e_grid = (int64_t)sm_count() * ((mode == 1) ? 2 : 24);
+  const size_t e_smem = (mode == 1) ? (size_t)tb->n_z * sizeof(double) : 0;
+  if (want_epoch) {
+    Q.want_units = 1; Q.un0 = slot->un0; Q.ucnt = slot->ucnt; Q.n_blocks = n_prep;
+    A.un0 = slot->un0; A.ucnt = slot->ucnt;
+    int64_t C = (4 * e_grid + n_pv - 1) / n_pv;
+    A.unit_chunks = (int)(C < 1 ? 1 : (C > 4096 ? 4096 : C));
+    A.base_added = (dtype == kDtypeChi2) ? 1 : 0;
+  }
   if (n_prep > 0) {
     // an ordinary launch: ordered behind whatever the caller enqueued before (the kernel that wrote d_params, the fill that
     // zeroed d_status), so it and its dependent below see the caller's data
@@ -319,7 +339,7 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
     else prep_kernel<1><<<n_prep, kThreads, 0, st>>>(A, Q);
     g_launches.fetch_add(1);
     A.prep = 1;
-    A.pvcache = want_rec ? slot->pv : nullptr;
+    A.pvcache = (want_rec || want_epoch) ? slot->pv : nullptr;
     A.order = want_order ? slot->order : nullptr;
     A.range = want_axis ? 1 : 0;
   }
@@ -335,6 +355,35 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = grid; cfg.blockDim = dim3(kThreads); cfg.dynamicSmemBytes = 0; cfg.stream = st;
   cfg.attrs = pdl_attr; cfg.numAttrs = A.prep ? 1 : 0;
+  if (want_epoch) {
+    cudaLaunchConfig_t ecfg = cfg;
+    ecfg.gridDim = dim3((unsigned)e_grid);
+    ecfg.blockDim = dim3((unsigned)e_nt);
+    ecfg.dynamicSmemBytes = e_smem;
+    ecfg.numAttrs = 1;
+    const bool ev2 = (n_t % 2 == 0) && (dtype == kDtypeChi2 || reinterpret_cast<uintptr_t>(d_flux) % 16 == 0);
+    cudaError_t e_err = cudaSuccess;
+#define PT_EPOCH(M, NTT, VV, S, T)                                                                                  \
+  do {                                                                                                              \
+    if (e_smem > 48 * 1024)                                                                                         \
+      e_err = cudaFuncSetAttribute(epoch_kernel<M, NTT, VV, S, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)e_smem); \
+    if (e_err == cudaSuccess) e_err = cudaLaunchKernelEx(&ecfg, epoch_kernel<M, NTT, VV, S, T>, A);                 \
+  } while (0)
+#define PT_EPOCH_T(M, NTT, T)                                                \
+  do {                                                                       \
+    if (ev2) { if (s1) PT_EPOCH(M, NTT, true, true, T); else PT_EPOCH(M, NTT, true, false, T); } \
+    else { if (s1) PT_EPOCH(M, NTT, false, true, T); else PT_EPOCH(M, NTT, false, false, T); }   \
+  } while (0)
+    if (mode == 0) {
+      if (dtype == PT_F64) PT_EPOCH_T(0, 32, double); else if (dtype == PT_F32) PT_EPOCH_T(0, 32, float); else PT_EPOCH_T(0, 32, Chi2);
+    } else {
+      if (dtype == PT_F64) PT_EPOCH_T(1, 512, double); else if (dtype == PT_F32) PT_EPOCH_T(1, 512, float); else PT_EPOCH_T(1, 512, Chi2);
+    }
+#undef PT_EPOCH_T
+#undef PT_EPOCH
+    g_launches.fetch_add(1);
+    A.epoch = 1;
+  }
 #define PT_LAUNCH(M, VV, P, S, T) cudaLaunchKernelEx(&cfg, flux_kernel<M, VV, P, S, T>, A)
 #define PT_LAUNCH_S(M, VV, P, T)                             \
   do {                                                       \
