@@ -233,7 +233,10 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? 24 : 2)) epoch_kernel(const __
       const double c0 = r.coef[0], c1 = r.coef[1], c2 = r.coef[2];
       // batches of Be <= 31 epochs (lane = epoch; one more lane looks at the epoch in front of the batch)
       const uint32_t nE = E1 - E0;
-      uint32_t Be = (nwp == 1) ? 31u : (nE + 3u * nwp - 1u) / (3u * nwp);
+#ifndef PT_BE_DIV
+#define PT_BE_DIV 5u
+#endif
+      uint32_t Be = (nwp == 1) ? 31u : (nE + PT_BE_DIV * nwp - 1u) / (PT_BE_DIV * nwp);
       Be = Be < 4u ? 4u : (Be > 31u ? 31u : Be);
       const int nbat = (int)((nE + Be - 1u) / Be);
       double chi = 0.0;
