@@ -29,8 +29,8 @@
 //   A row that is always in the window, or whose epochs are denser than one per eight exposures, is cut into chunks of
 //   kChunkLen exposures instead of epochs (every exposure evaluated); a row that never transits is all fill; a bad row NaN.
 //
-// If prep_kernel finds the axis not ascending (or not finite) this kernel returns at once and the general flux kernel
-// (pt_flux.cuh), launched behind it, does the work.
+// If prep_kernel finds the axis not ascending (or not finite), every row is cut into chunks: exact for any order of the
+// times, only slow.
 #pragma once
 #include "pt_flux.cuh"
 
@@ -179,9 +179,10 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? 24 : 2)) epoch_kernel(const __
     for (int i = lane; i < kAccRing; i += 32) W.acc[i] = 0;
     __syncthreads();
   }
-  asm volatile("griddepcontrol.launch_dependents;");   // the fallback kernel behind this one may be scheduled: it waits
   asm volatile("griddepcontrol.wait;" ::: "memory");   // prep_kernel's slot (records, units, order, axis flag) is complete
-  if (*((volatile const unsigned long long*)(A.sched + kW_Flags)) & kSlotUnsorted) return;   // the general kernel takes over
+  // an axis that is not ascending (or not finite) has no index ranges: every row is then cut into chunks and every exposure
+  // evaluated (slow, but exact for any order of the times: an exposure outside the transit evaluates to flux 1)
+  const bool unsorted = *((volatile const unsigned long long*)(A.sched + kW_Flags)) & kSlotUnsorted;
   const int C = A.unit_chunks;
   const unsigned long long n_units = (unsigned long long)A.n_pv * (unsigned long long)C;
   const int n_t = (int)A.n_t;
@@ -197,7 +198,8 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? 24 : 2)) epoch_kernel(const __
     const int64_t j = (int64_t)(ticket / (unsigned long long)C);
     const int c = (int)(ticket - (unsigned long long)j * C);
     const int64_t pv = A.order ? (int64_t)__ldg(A.order + j) : j;
-    const uint32_t ucnt = __ldg(A.ucnt + pv);
+    uint32_t ucnt = __ldg(A.ucnt + pv);
+    if (unsorted && ucnt != 0u) ucnt = kUnitChunks | (uint32_t)((n_t + kChunkLen - 1) / kChunkLen);
     const double un0 = __ldg(A.un0 + pv);
     {
       const double* src = reinterpret_cast<const double*>(A.pvcache + pv);
@@ -337,7 +339,7 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? 24 : 2)) epoch_kernel(const __
           // supersampled: items y = x n_ss + s, 32 per round; segmented fixed-point sum per exposure, carried in W.acc
           const long long n_items = (long long)n_exp * n_ss;
           for (long long y0 = 0; y0 < n_items; y0 += 32) {
-            const int x0 = (int)(y0 / n_ss);
+            const int x0 = (n_items < 0x7fffffffLL) ? (int)((uint32_t)y0 / (uint32_t)n_ss) : (int)(y0 / n_ss);
             const int v = (int)(y0 - (long long)x0 * n_ss) + lane;          // < n_ss + 32
             const int dx = (n_ss >= 32) ? (v >= n_ss ? 1 : 0) : (int)(((uint32_t)v * ss_magic) >> 16);
             const int x = x0 + dx, sub = v - dx * n_ss;

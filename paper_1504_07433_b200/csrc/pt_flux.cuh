@@ -105,7 +105,6 @@ struct FluxArgs {
   const PvRec* pvcache;        // single passband, few parameter vectors: records precomputed by prep_kernel (else NULL)
   const uint32_t* order;       // global mode: row order of the tiles written by prep_kernel (heaviest rows first / rows sorted
                                // by k̂ for the table), or NULL = index order
-  int epoch;                   // 1: this launch runs behind the epoch kernel and only acts if the axis turned out unsorted
   int per_pv;                  // 1: warps stay on one parameter vector and take its tiles from its own counter (n_pv small)
   int prep;                    // 1: launched as a programmatic dependent of prep_kernel: wait for it before reading the slot
   int range;                   // 1: one shared time axis; if prep_kernel found it ascending and finite, out-of-window
@@ -845,7 +844,6 @@ __global__ void __launch_bounds__(kThreads, PT_MIN_BLOCKS) flux_kernel(const __g
   // The slot (order, records, flags) is written by prep_kernel, whose programmatic dependent this grid is.
   if (A.prep) asm volatile("griddepcontrol.wait;" ::: "memory");
   const bool sorted_axis = A.range && !(*((volatile const unsigned long long*)(A.sched + kW_Flags)) & kSlotUnsorted);
-  if (A.epoch && sorted_axis) return;   // the epoch kernel in front of this one did the whole launch (and cleaned the slot)
   const int tpp = A.tiles_per_pv;
   int64_t pv_cur = 0, last_pv = -1;
   int chunk_cur = 0, last_ring = -1;
@@ -1161,7 +1159,8 @@ __device__ __forceinline__ void pv_units(const PvConst& c, double T_first, doubl
   const double pad = 0x1p-49 * (fabs(x0) + fabs(x1) + 2.0);
   const double a = ceil(x0 - c.ex_hi - pad), b = floor(x1 - c.ex_lo + pad);
   const double m = b - a + 1.0;
-  if (!(m >= 1.0)) return;                                  // no epoch on the axis (or a non-finite axis: never used then)
+  if (!(m == m) || fabs(m) > 1.0e300) { *cnt = chunks; return; }   // non-finite axis ends: the row is cut into chunks
+  if (!(m >= 1.0)) return;                                  // no epoch on the axis
   if (m > 0.125 * (double)n_t + 2.0 || m > 1.0e9) { *cnt = chunks; return; }
   *n0 = a; *cnt = (uint32_t)m;
 }

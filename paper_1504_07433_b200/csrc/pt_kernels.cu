@@ -300,7 +300,7 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   //   order    global tile counter: heaviest rows first (mode 2), or rows by k̂ for the interpolated model
   //   baseline fused likelihood
   const bool want_rec = n_pb == 1 && pb_view < 0 && n_pv <= kPvCacheMax && A.n_tiles >= 8 * n_pv;
-  const bool want_axis = t_stride_pv == 0 && n_t >= 512 && (double)n_pv * (double)n_t >= (double)PT_RANGE_MIN;
+  const bool want_axis = t_stride_pv == 0 && n_t >= 2048 && (double)n_pv * (double)n_t >= (double)PT_RANGE_MIN;
   // epoch kernel: one passband on one shared axis that prep_kernel checks; it does the whole launch if the axis is ascending,
   // else the general kernel launched behind it does
   const bool want_epoch = want_axis && n_pb == 1 && pb_view < 0 && n_pv <= kPvCacheMax && n_t < 0x7fffff00LL &&
@@ -382,7 +382,9 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
 #undef PT_EPOCH_T
 #undef PT_EPOCH
     g_launches.fetch_add(1);
-    A.epoch = 1;
+    const cudaError_t err2 = cudaGetLastError();
+    slot_release(ticket, st);
+    return (e_err == cudaSuccess && err2 == cudaSuccess) ? PT_OK : PT_ERR_CUDA;
   }
 #define PT_LAUNCH(M, VV, P, S, T) cudaLaunchKernelEx(&cfg, flux_kernel<M, VV, P, S, T>, A)
 #define PT_LAUNCH_S(M, VV, P, T)                             \
