@@ -48,7 +48,16 @@ extern "C" {
 #endif
 
 enum { PT_OK = 0, PT_ERR_NULL = 1, PT_ERR_SIZE = 2, PT_ERR_DTYPE = 3, PT_ERR_TABLE = 4, PT_ERR_CUDA = 5 };
-enum { PT_F64 = 0, PT_F32 = 1 };                          /* storage type of the flux / of a table (arithmetic is fp64) */
+enum { PT_F64 = 0, PT_F32 = 1, PT_F32S = 2 };
+/* Flux dtype.  PT_F64: fp64 arithmetic, double output.  PT_F32: the fp32 VARIANT of BASELINE.json (gate 2e-6 absolute;
+ * SURVEY §8(c)-4 H5): float output and fp32 ARITHMETIC from the folded phase on — orbit, case split, λe, λd*, ηd, combine —
+ * on the FP32 pipe; the subsample time and the phase fold stay fp64 (a time of ~1e3 d resolves 1e-4 d in fp32).  A
+ * parameter vector for which fp32 cannot hold the gate — limb-darkening coefficients that would carry the measured
+ * worst-case errors of the fp32 basis functions (λd*: 9.5e-7) beyond 1.6e-6 in flux, k > 0.7, a/R* > 50 or e > 0.85 —
+ * is evaluated in fp64 and only stored as float (a per-vector decision).  fp32 arithmetic exists in pt_ma_quad_exact
+ * with one passband; elsewhere (several passbands, pt_ma_quad_exact_pbk, pt_ma_quad_interp) PT_F32 means PT_F32S.
+ * PT_F32S: fp64 arithmetic, float storage (half the output traffic).
+ * Table dtype (pt_table.dtype, pt_ma_table_build): PT_F64 or PT_F32 = storage type of the nodes (computed in fp64). */
 enum { PT_ST_BAD_PARAM = 1, PT_ST_K_OUT_OF_TABLE = 2 };   /* bits OR-ed into d_status[0] */
 
 /* Interpolation table descriptor (host struct holding a device pointer).  Layout [n_k][n_z][n_fn], n_fn = 3
@@ -70,10 +79,7 @@ int pt_orbit_z(const double* d_times, int64_t n_t, int64_t t_stride_pv, const do
                int32_t n_pb, int32_t n_ss, double t_exp, double* d_z, void* stream);
 
 /* S0-S7: exact quadratic Mandel–Agol flux (Eq. 13 with P:L143).
- *   dtype  PT_F64: d_flux is double.  PT_F32: d_flux is float (the fp32 variant of BASELINE.json, gate 2e-6 abs): the
- *          arithmetic stays fp64 up to the store, because the closed forms lose 2-3 digits to cancellation near the
- *          contacts and for small k, which fp32 cannot afford at 2e-6 (R18); what fp32 buys is half the
- *          output traffic, which is what bounds the out-of-transit and interpolated paths.
+ *   dtype  PT_F64: d_flux is double.  PT_F32 / PT_F32S: d_flux is float (see the enum above).
  *   d_flux [n_pv][n_pb][n_t], time fastest.   d_status: NULL or 2 x int32 (see above). */
 int pt_ma_quad_exact(const double* d_times, int64_t n_t, int64_t t_stride_pv, const double* d_params, int64_t n_pv,
                      int32_t n_pb, int32_t n_ss, double t_exp, int32_t dtype, void* d_flux, int32_t* d_status,

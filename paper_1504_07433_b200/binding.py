@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpt_b200.so")
 
 PT_OK, PT_ERR_NULL, PT_ERR_SIZE, PT_ERR_DTYPE, PT_ERR_TABLE, PT_ERR_CUDA = range(6)
-PT_F64, PT_F32 = 0, 1
+PT_F64, PT_F32, PT_F32S = 0, 1, 2
 PT_ST_BAD_PARAM, PT_ST_K_OUT_OF_TABLE = 1, 2
 _ERR = {1: "PT_ERR_NULL", 2: "PT_ERR_SIZE", 3: "PT_ERR_DTYPE", 4: "PT_ERR_TABLE", 5: "PT_ERR_CUDA"}
 
@@ -118,13 +118,17 @@ def pt_orbit_z(times: torch.Tensor, params: torch.Tensor, n_pb: int = 1, n_ss: i
 
 def pt_ma_quad_exact(times: torch.Tensor, params: torch.Tensor, n_pb: int = 1, n_ss: int = 1, t_exp: float = 0.0,
                      dtype: torch.dtype = torch.float64, out: Optional[torch.Tensor] = None,
-                     status: Optional[torch.Tensor] = None) -> torch.Tensor:
-    """Exact quadratic Mandel–Agol flux [n_pv][n_pb][n_t] (include/pt.h: pt_ma_quad_exact)."""
+                     status: Optional[torch.Tensor] = None, fp32_store_only: bool = False) -> torch.Tensor:
+    """Exact quadratic Mandel–Agol flux [n_pv][n_pb][n_t] (include/pt.h: pt_ma_quad_exact).
+    float32 output selects PT_F32 (fp32 arithmetic from the folded phase on), or PT_F32S with fp32_store_only."""
     times, params, n_pv, n_t, stride = _marshal(times, params, n_pb)
     if out is None:
         out = torch.empty((n_pv, n_pb, n_t), dtype=dtype, device=times.device)
+    code = _dtype_code(out.dtype)
+    if code == PT_F32 and fp32_store_only:
+        code = PT_F32S
     _check(lib().pt_ma_quad_exact(times.data_ptr(), n_t, stride, params.data_ptr(), n_pv, n_pb, n_ss, float(t_exp),
-                                  _dtype_code(out.dtype), out.data_ptr(),
+                                  code, out.data_ptr(),
                                   status.data_ptr() if status is not None else None, _stream()), "pt_ma_quad_exact")
     return out
 

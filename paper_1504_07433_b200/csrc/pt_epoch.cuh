@@ -305,6 +305,9 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? 24 : 2)) epoch_kernel(const __
           } else if (MODE == 1) {
             return ma_dec_noinline(khat, zs, c0, c1, c2);
           } else {
+            if constexpr (kF32Capable<OutT>) {
+              if (r.f.use) return (double)ma_dec32(r.f, (float)zs);
+            }
             const Basis b = ma_basis(khat, zs);
             return fma(c2, b.ed, fma(c1, b.ld, c0 * b.le));
           }
@@ -329,8 +332,8 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? 24 : 2)) epoch_kernel(const __
             const int e = e1; const double t = t1; const bool act = a1;
             if (q + 1 < R) fetch(q + 1, e1, t1, a1);       // the next round's times are in flight during this one
             if (act) {
-              const double zs = orbit_z_signed(r.c, fold_phase(t, r.c.t0, r.c.P, r.c.invP, slow_div));
-              const bool in = zs >= 0.0 && zs < 1.0 + khat;
+              bool in;
+              const double zs = sample_z<OutT>(r, fold_phase(t, r.c.t0, r.c.P, r.c.invP, slow_div), in);
               const double dec = in ? decrement(zs) : 0.0;
               if (in || !kIsChi2<OutT>) emit1<OutT>(A, row, (uint32_t)e, dec, chi);
             }
@@ -349,8 +352,9 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? 24 : 2)) epoch_kernel(const __
             if (act) {
               const double t = ldg_keep(A.times + e, pol);
               const double ts = __dadd_rn(t, sub < kOffTable ? s_off[sub] : subsample_offset(sub, n_ss, A.t_exp));
-              const double zs = orbit_z_signed(r.c, fold_phase(ts, r.c.t0, r.c.P, r.c.invP, slow_div));
-              if (zs >= 0.0 && zs < 1.0 + khat) fx = __double2ll_rn(decrement(zs) * r.acc_scale);
+              bool in;
+              const double zs = sample_z<OutT>(r, fold_phase(ts, r.c.t0, r.c.P, r.c.invP, slow_div), in);
+              if (in) fx = __double2ll_rn(decrement(zs) * r.acc_scale);
             }
             const int sid = act ? x : -1 - lane;
             for (int o = 1; o < G; o <<= 1) {

@@ -32,6 +32,7 @@
 #include "../../include/pt.h"
 #include "pt_basis.cuh"
 #include "pt_orbit.cuh"
+#include "pt_basis32.cuh"
 
 namespace pt {
 
@@ -49,7 +50,7 @@ constexpr int kExpQ = PT_UNROLL > 4 ? 1024 : 512;      // exposure ring: >= 32*k
 constexpr int kItemQ = 64;      // item ring: at most 31 left over + 32 new per z-round
 constexpr int kSlots = 64;      // pending-exposure records (supersampled path): <= 31 + 32 alive
 constexpr int kPvRing = 4;      // parameter-vector records a warp keeps alive (single-passband path)
-constexpr int kCoefCache = 32;  // passbands whose combine coefficients are cached per warp (multi-passband path)
+constexpr int kCoefCache = 24;  // passbands whose combine coefficients are cached per warp (multi-passband path)
 constexpr int kMaxTileLen = 32768;
 constexpr int kRemBias = 1 << 24;
 constexpr int kSchedHead = 8;   // words of a scheduler slot in front of the per-parameter-vector tickets
@@ -113,6 +114,8 @@ struct FluxArgs {
   const double* un0;           // [n_pv] first transit epoch on the axis (units in epoch mode)
   const uint32_t* ucnt;        // [n_pv] number of units; kUnitChunks set: the row is cut into chunks of kChunkLen exposures
   int unit_chunks;             // work units per row: unit (row, c) owns the epochs [c cnt/C, (c+1) cnt/C) and the gaps in front of them
+  int f32a;                    // 1: fp32 ARITHMETIC from the folded phase on (PT_F32; float output, single passband) where
+                               // the parameter vector allows it (pt_basis32.cuh: f32_ok)
   int base_added;              // fused likelihood: prep_kernel already left the baseline in chi2[]
   // supersample accumulation (fixed point)
   int fx_bits;             // 61 - ceil(log2 n_ss): a sum of n_ss values below 2^eb fits an int64 at scale 2^(fx_bits-eb)
@@ -143,6 +146,7 @@ struct PvRec {
   double fk;               // table: fractional k index
   int ik;                  // table: lower k index
   int use_table;
+  PvF32 f;                 // fp32 copies for the fp32-arithmetic variant (f.use)
 };
 
 struct Slot {              // a supersampled exposure with subsamples still in the item queue
@@ -331,6 +335,35 @@ __device__ __forceinline__ Basis eval_basis(const FluxArgs& A, const PvRec& r, d
   return ma_basis(r.c.khat, z);
 }
 
+// The fp32-arithmetic variant exists in the kernels that store fp32 flux; whether a parameter vector takes it is decided
+// once per vector (PvRec::f.use), so the branch below is uniform over a tile.
+template <typename OutT> constexpr bool kF32Capable = std::is_same<OutT, float>::value;
+
+// Signed separation of a sample at pinned folded phase ph, and whether it is in transit (0 <= z < 1 + k̂).
+template <typename OutT>
+__device__ __forceinline__ double sample_z(const PvRec& r, double ph, bool& in) {
+  if constexpr (kF32Capable<OutT>) {
+    if (r.f.use) {
+      const float zf = orbit_z_signed32(r.f, r.c.Mtr, r.c.flags & PV_CIRCULAR, ph);
+      in = zf >= 0.0f && zf < 1.0f + r.f.khat;
+      return (double)zf;
+    }
+  }
+  const double zs = orbit_z_signed(r.c, ph);
+  in = zs >= 0.0 && zs < 1.0 + r.c.khat;
+  return zs;
+}
+
+// Combined decrement coef0 λe + coef1 λd* + coef2 ηd of an in-transit sample (single passband).
+template <int MODE, typename OutT>
+__device__ __forceinline__ double sample_dec(const FluxArgs& A, const PvRec& r, double z) {
+  if constexpr (kF32Capable<OutT>) {
+    if (r.f.use) return (double)ma_dec32(r.f, (float)z);
+  }
+  const Basis b = eval_basis<MODE>(A, r, z);
+  return fma(r.coef[2], b.ed, fma(r.coef[1], b.ld, r.coef[0] * b.le));
+}
+
 // 2^s as a double, s clamped to the normal range.
 __device__ __forceinline__ double pow2i(int s) {
   s = min(max(s, -1000), 1000);
@@ -402,6 +435,7 @@ __device__ __noinline__ void tile_setup(const FluxArgs& A, WarpState& ws, int ri
     r.row = row;
     r.ik2 = ik2;
     r.use_table = 0;
+      r.f.use = 0;
   }
   if (c.flags & PV_BAD) {
     if (chunk == 0 && lane == 0 && A.status) {
@@ -424,6 +458,12 @@ __device__ __noinline__ void tile_setup(const FluxArgs& A, WarpState& ws, int ri
       r.coef[0] = c0; r.coef[1] = c1; r.coef[2] = c2;
       r.acc_scale = pow2i(A.fx_bits - eb);
       r.acc_inv = pow2i(eb - A.fx_bits) * A.inv_nss;
+      // fp32-arithmetic variant: large a/R* or e amplify the fp32 rounding of the orbit beyond the gate
+      r.f.use = (A.f32a && MODE == 0 && f32_ok(khat, c0, c1, c2) && c.a <= 50.0 && c.e <= 0.85) ? 1 : 0;
+      r.f.a = (float)c.a; r.f.cosi = (float)c.cosi; r.f.ci2 = (float)(c.cosi * c.cosi); r.f.e = (float)c.e;
+      r.f.sinw = (float)c.sinw; r.f.cosw = (float)c.cosw; r.f.rt1me2 = (float)c.rt1me2; r.f.sin_e = (float)c.sin_e;
+      r.f.cos_e = (float)c.cos_e; r.f.khat = (float)khat;
+      r.f.coef[0] = (float)c0; r.f.coef[1] = (float)c1; r.f.coef[2] = (float)c2;
     }
   } else {
     for (int j = lane; j < n_pb && j < kCoefCache; j += 32) {
@@ -496,10 +536,10 @@ __device__ PT_BASIS_INLINE void basis_round(const FluxArgs& A, WarpState& ws, Ss
     if (act) {
       ring = ss.slots[sid].ring;
       const PvRec& r = ws.pv[ring];
-      const Basis b = eval_basis<MODE>(A, r, ss.item_z[idx]);
       if (NPB1) {
-        v[0] = __double2ll_rn(fma(r.coef[2], b.ed, fma(r.coef[1], b.ld, r.coef[0] * b.le)) * r.acc_scale);
+        v[0] = __double2ll_rn(sample_dec<MODE, OutT>(A, r, ss.item_z[idx]) * r.acc_scale);
       } else {
+        const Basis b = eval_basis<MODE>(A, r, ss.item_z[idx]);
         v[0] = __double2ll_rn(b.le * A.fx_scale);
         v[NACC - 2] = __double2ll_rn(b.ld * A.fx_scale);
         v[NACC - 1] = __double2ll_rn(b.ed * A.fx_scale);
@@ -576,15 +616,15 @@ __device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, SsStat
   const int qhead = C.qhead;
   const uint32_t e = act ? ws.expq[(qhead + grp) & (kExpQ - 1)] : 0u;
   const double t = act ? __ldg(r.tb + e) : 0.0;
-  const double khat = r.c.khat;
   const bool slow_div = r.c.flags & PV_SLOWDIV;
   OutT* ob = (OutT*)r.ob;
   if (SS1) {
     // n_ss == 1: an exposure in the window is almost always in transit, so a second compaction would buy nothing; the
     // basis functions are evaluated right here, one exposure per lane, and the item queue stays empty.
     if (act) {
-      const double zs = orbit_z_signed(r.c, fold_phase(t, r.c.t0, r.c.P, r.c.invP, slow_div));
-      if (zs >= 0.0 && zs < 1.0 + khat) {
+      bool in_tr;
+      const double zs = sample_z<OutT>(r, fold_phase(t, r.c.t0, r.c.P, r.c.invP, slow_div), in_tr);
+      if (in_tr) {
         if (!NPB1 && MODE == 0 && A.pbk) {
           // exact per-passband-k mode (S§8(f) NEXT-2): one orbit evaluation, the basis functions once per passband at k_j
           double chi = 0.0;
@@ -603,9 +643,12 @@ __device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, SsStat
             emit<OutT>(A, r, (OutT*)r.ob + e, e, j, fma(c2, b.ed, fma(c1, b.ld, c0 * b.le)), chi);
           }
         } else {
-          const Basis b = eval_basis<MODE>(A, r, zs);
-          if (NPB1) finish_exposure<true, OutT>(A, ws, r, e, fma(r.coef[2], b.ed, fma(r.coef[1], b.ld, r.coef[0] * b.le)), 0.0, 0.0, &chi_acc);
-          else finish_exposure<false, OutT>(A, ws, r, e, b.le, b.ld, b.ed, &chi_acc);
+          if (NPB1) {
+            finish_exposure<true, OutT>(A, ws, r, e, sample_dec<MODE, OutT>(A, r, zs), 0.0, 0.0, &chi_acc);
+          } else {
+            const Basis b = eval_basis<MODE>(A, r, zs);
+            finish_exposure<false, OutT>(A, ws, r, e, b.le, b.ld, b.ed, &chi_acc);
+          }
         }
       } else {
         store_one<NPB1, OutT>(ob + e, A.n_t, n_pb);
@@ -626,8 +669,7 @@ __device__ PT_EXPAND_INLINE void expand(const FluxArgs& A, WarpState& ws, SsStat
       double zs = 0.0;
       if (act && s < n_ss) {
         const double ts = __dadd_rn(t, multi ? subsample_offset(s, n_ss, A.t_exp) : L.off0);
-        zs = orbit_z_signed(r.c, fold_phase(ts, r.c.t0, r.c.P, r.c.invP, slow_div));
-        p = zs >= 0.0 && zs < 1.0 + khat;
+        zs = sample_z<OutT>(r, fold_phase(ts, r.c.t0, r.c.P, r.c.invP, slow_div), p);
       }
       const unsigned m = __ballot_sync(0xffffffffu, p);
       int nalloc = 0;

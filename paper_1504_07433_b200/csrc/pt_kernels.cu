@@ -253,19 +253,22 @@ struct Chi2Args {
   const double* obs;
   const double* isig;
 };
-constexpr int kDtypeChi2 = 2;   // internal: d_flux is chi2[n_pv], `like` holds the observations
+constexpr int kDtypeChi2 = 100;   // internal: d_flux is chi2[n_pv], `like` holds the observations
 
 static int launch_flux(int mode, const pt_table* tb, const double* d_times, int64_t n_t, int64_t t_stride_pv,
                        const double* d_params, int64_t n_pv, int n_pb, int n_ss, double t_exp, int dtype, void* d_flux,
                        int32_t* d_status, cudaStream_t st, const Chi2Args* like = nullptr, int pb_view = -1, int n_pb_row = 0) {
   int rc = check_common(d_times, d_params, d_flux, n_t, t_stride_pv, n_pv, n_pb, n_ss);
   if (rc) return rc;
-  if (dtype != PT_F64 && dtype != PT_F32 && !(dtype == kDtypeChi2 && like)) return PT_ERR_DTYPE;
+  if (dtype != PT_F64 && dtype != PT_F32 && dtype != PT_F32S && !(dtype == kDtypeChi2 && like)) return PT_ERR_DTYPE;
+  const bool f32a = (dtype == PT_F32) && mode == 0 && n_pb == 1 && pb_view == -1;   // fp32 arithmetic where the kernels have it
+  if (dtype == PT_F32S) dtype = PT_F32;                   // from here on: the storage type
   FluxArgs A{};
   A.times = d_times; A.n_t = n_t; A.t_stride_pv = t_stride_pv; A.params = d_params; A.n_pv = n_pv;
   A.n_pb = n_pb; A.n_ss = n_ss; A.t_exp = t_exp; A.flux = d_flux; A.status = d_status;
   A.row_stride = 6 + 3 * (int64_t)n_pb; A.pb_first = 0; A.flux_pv_stride = (int64_t)n_pb * n_t; A.flux_off = 0;
   A.pbk = (pb_view == -2) ? 1 : 0;
+  A.f32a = f32a ? 1 : 0;
   if (pb_view >= 0) {   // single-passband view of passband `pb_view` in rows of n_pb_row passbands
     A.row_stride = 6 + 3 * (int64_t)n_pb_row; A.pb_first = pb_view;
     A.flux_pv_stride = (int64_t)n_pb_row * n_t; A.flux_off = (int64_t)pb_view * n_t;
@@ -552,7 +555,7 @@ static int run_host(int mode, const pt_table* tb, const double* h_times, int64_t
   // every argument error is reported before anything is allocated or enqueued
   int rc = check_common(h_times, h_params, h_flux, n_t, t_stride_pv, n_pv, n_pb, n_ss);
   if (rc) return rc;
-  if (dtype != PT_F64 && dtype != PT_F32) return PT_ERR_DTYPE;
+  if (dtype != PT_F64 && dtype != PT_F32 && dtype != PT_F32S) return PT_ERR_DTYPE;
   if (mode == 1 && !table_ok(tb)) return PT_ERR_TABLE;
   if (plan_tiles(n_pv, n_t, sm_count()).tile_len == 0) return PT_ERR_SIZE;
   int dev = 0;

@@ -193,6 +193,54 @@ def test_fp32_variant(pt, oracle, cfg):
     assert np.abs(f.astype(np.float64) - ora_exact(oracle, w)).max() <= TOL32
 
 
+def test_fp32_store_only_mode_is_fp64_arithmetic(pt, oracle):
+    # PT_F32S: fp64 arithmetic, float storage: equals the fp64 flux rounded to float
+    w = inputs.config5(oz64(oracle), n_pv=64, n_t=512)
+    f64 = gpu_exact(pt, w)
+    f = pt.pt_ma_quad_exact(dev(w.times), dev(w.params), dtype=torch.float32, fp32_store_only=True)
+    torch.cuda.synchronize()
+    assert np.array_equal(f.cpu().numpy(), f64.astype(np.float32))
+
+
+@pytest.mark.parametrize("u", [(0.4, 0.2), (0.0, 0.0), (0.9, -0.1), (0.0, 1.0)])
+def test_fp32_arith_h5_grid(pt, oracle, u):
+    # the region where fp32 λd* is worst — small k, close to the inner contact — on an explicit grid:
+    # k in {0.01, 0.05, 0.1, 0.4}, |z - (1-k)| in {1e-6, 1e-4, 1e-2}, plus z = k, z -> 0 and the outer contact.
+    # Circular orbit seen edge-on (i = π/2): z(t) = a |sin(2π t / P)|, so a wanted z is the time P/(2π) asin(z/a).
+    # (0, 1) is an extreme law whose coefficients send the row to fp64 arithmetic (f32_ok): it must hold the gate too.
+    a, P = 10.0, 3.0
+    rows, times = [], []
+    for k in (0.01, 0.05, 0.1, 0.4):
+        zs = [1e-7, 0.5 * k, k, k * (1 + 1e-5), 0.5, 1.0 + k - 1e-4, 1.0 + k - 1e-2]
+        for d in (1e-6, 1e-4, 1e-2):
+            zs += [1.0 - k - d, 1.0 - k + d]
+        zs.append(1.0 - k)
+        zs = np.array(zs)
+        times.append(P / (2 * np.pi) * np.arcsin(zs / a))
+        rows.append([0.0, P, a, 0.5 * np.pi, 0.0, 0.0, k, u[0], u[1]])
+    params = np.array(rows)
+    t = np.array(times)
+    f = pt.pt_ma_quad_exact(dev(t), dev(params), dtype=torch.float32)
+    torch.cuda.synchronize()
+    ref = oracle.ma_quad_exact(t, params, prec="f128")
+    err = np.abs(f.cpu().numpy().astype(np.float64) - ref)
+    assert err.max() <= TOL32, (err.max(), np.unravel_index(err.argmax(), err.shape))
+
+
+def test_fp32_arith_dense_eccentric_and_shared_axis(pt, oracle):
+    # the two kernels that have the fp32 path: per-row times (eccentric, n_ss = 1) and the shared ascending axis (epoch
+    # kernel, supersampled), both at sizes that span many tiles
+    w = inputs.dense_transit(n_pv=256, n_t=1024)
+    f = gpu_exact(pt, w, dtype=torch.float32)
+    err = np.abs(f.astype(np.float64) - ora_exact(oracle, w, "f64")).max()
+    assert err <= TOL32, err
+    w = inputs.config2(n_pv=48, n_t=6000)
+    f = gpu_exact(pt, w, dtype=torch.float32)
+    err = np.abs(f.astype(np.float64) - ora_exact(oracle, w, "f64")).max()
+    assert err <= TOL32, err
+    assert (f == 1.0).mean() > 0.9                       # out of transit: exactly 1
+
+
 # ------------------------------------------------------------------------------------------- table + interpolated path
 def _table_cfg(small=True):
     return dict(k_min=0.05, k_max=0.25, n_k=41, z_max=1.25, n_z=1251) if small else inputs.config4(1, 1).table
