@@ -53,7 +53,7 @@ enum { PT_F64 = 0, PT_F32 = 1, PT_F32S = 2 };
  * SURVEY §8(c)-4 H5): float output and fp32 ARITHMETIC from the folded phase on — orbit, case split, λe, λd*, ηd, combine —
  * on the FP32 pipe; the subsample time and the phase fold stay fp64 (a time of ~1e3 d resolves 1e-4 d in fp32).  A
  * parameter vector for which fp32 cannot hold the gate — limb-darkening coefficients that would carry the measured
- * worst-case errors of the fp32 basis functions (λd*: 9.5e-7) beyond 1.6e-6 in flux, k > 0.7, a/R* > 50 or e > 0.85 —
+ * worst-case errors of the fp32 basis functions (λd*: 8e-7) beyond 1.75e-6 in flux, k > 0.7, a/R* > 50 or e > 0.85 —
  * is evaluated in fp64 and only stored as float (a per-vector decision).  fp32 arithmetic exists in pt_ma_quad_exact
  * with one passband; elsewhere (several passbands, pt_ma_quad_exact_pbk, pt_ma_quad_interp) PT_F32 means PT_F32S.
  * PT_F32S: fp64 arithmetic, float storage (half the output traffic).

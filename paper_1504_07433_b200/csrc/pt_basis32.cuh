@@ -15,6 +15,11 @@
 
 namespace pt {
 
+#ifndef PT_F32_NTHR
+#define PT_F32_NTHR 1.2f   // |n| below which cK K + cP Π is evaluated as (cK+cP) K + cP (Π-K): in fp32 the rewrite pays up to
+                           // |n| ~ 1.2 (worst λd* error over k: 9.0e-7 with 0.5 as in fp64, 7.8e-7 with 1.2, 8.0e-7 with 1.5, 8.6e-7 with 2)
+#endif
+
 struct Basis32 {
   float le, ld, ed;
   float ld_err;            // bound on the absolute error of ld
@@ -171,7 +176,7 @@ __device__ __forceinline__ Basis32 ma_basis32(float p, float z) {
       cE = 4.0f * pz * w7;
       pref = 0.0353677651f * rpz;
       const float bm1 = sm1 * sp1;
-      if (oma < 0.5f * a) {
+      if (oma < PT_F32_NTHR * a) {
         cK = fmaf(-bm1, 2.0f * b + a - 3.0f, -3.0f * q * fmaf(a, bm1, oma) * (rd * rd));
         a2 = 0.0f;
         b2 = -oma * (rd * rd) * ad;
@@ -187,7 +192,7 @@ __device__ __forceinline__ Basis32 ma_basis32(float p, float z) {
       cE = oma * w7;
       pref = 0.0707355303f * roma;
       const float pz4 = 4.0f * p * z;
-      if (pz4 < 0.5f * d * d) {
+      if (pz4 < PT_F32_NTHR * d * d) {
         cK = oma * fmaf(-3.0f * q, rd * rd, -sm1 * sp1);
         a2 = 0.0f;
         b2 = -pz4 * (rd * rd) * (ad * rs);
@@ -213,11 +218,16 @@ static_assert(sizeof(PvF32) % 8 == 0, "records are copied as doubles");
 
 // Worst absolute errors of ma_basis32 against the fp64 functions, measured over k in [0.005, 0.7] and z in [0, 1+k] with
 // 4e5 points per k, a quarter of them within 1e-7 ... 1e-2 of the inner contact (profiles/r2_fp32_variant.md): λe 9e-8,
-// λd* 9e-7 (reached within 1e-5 of the inner contact for k ~ 0.1; 3-4e-7 over the bulk), ηd 8e-8.  A parameter vector
-// whose limb-darkening coefficients would carry them beyond 1.6e-6 in flux (gate: 2e-6), or with k > 0.7, keeps fp64
-// arithmetic: the decision is uniform per parameter vector, so no warp diverges over it.
-__device__ __forceinline__ bool f32_ok(double khat, double c0, double c1, double c2) {
-  return khat <= 0.7 && (fabs(c0) * 9.0e-8 + fabs(c1) * 9.5e-7 + fabs(c2) * 8.0e-8) <= 1.6e-6;
+// λd* 7.8e-7 (k ~ 0.17 within 1e-4 of the inner contact; 2-3e-7 over the bulk), ηd 8e-8.  A parameter vector whose
+// limb-darkening coefficients would carry them beyond 1.75e-6 in flux (gate: 2e-6), or with k > 0.7, keeps fp64
+// arithmetic: the decision is uniform per parameter vector, so no warp diverges over it (NaN parameters compare false).
+// Large a/R* or e amplify the fp32 rounding of the orbit beyond the gate as well.  One function, so that every kernel
+// takes the same decision for a row: from the raw parameters (k, u1, u2, a/R*, e) of a single-passband row.
+__device__ __forceinline__ bool f32_ok(double k, double u1, double u2, double a, double e) {
+  const double cj = u1 + 2.0 * u2;
+  const double gN = 1.0 / (1.0 - u1 / 3.0 - u2 / 6.0);
+  const double c0 = gN * (1.0 - cj), c1 = gN * cj, c2 = gN * u2;
+  return k <= 0.7 && a <= 50.0 && e <= 0.85 && (fabs(c0) * 9.0e-8 + fabs(c1) * 8.0e-7 + fabs(c2) * 8.0e-8) <= 1.75e-6;
 }
 
 // Eccentric anomaly from mean anomaly M in (-π, π] in fp32: the starter of pt_orbit.cuh, Newton steps with a full (cheap)

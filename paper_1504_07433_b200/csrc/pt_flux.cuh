@@ -458,8 +458,7 @@ __device__ __noinline__ void tile_setup(const FluxArgs& A, WarpState& ws, int ri
       r.coef[0] = c0; r.coef[1] = c1; r.coef[2] = c2;
       r.acc_scale = pow2i(A.fx_bits - eb);
       r.acc_inv = pow2i(eb - A.fx_bits) * A.inv_nss;
-      // fp32-arithmetic variant: large a/R* or e amplify the fp32 rounding of the orbit beyond the gate
-      r.f.use = (A.f32a && MODE == 0 && f32_ok(khat, c0, c1, c2) && c.a <= 50.0 && c.e <= 0.85) ? 1 : 0;
+      r.f.use = (A.f32a && MODE == 0 && f32_ok(khat, u1, u2, c.a, c.e)) ? 1 : 0;
       r.f.a = (float)c.a; r.f.cosi = (float)c.cosi; r.f.ci2 = (float)(c.cosi * c.cosi); r.f.e = (float)c.e;
       r.f.sinw = (float)c.sinw; r.f.cosw = (float)c.cosw; r.f.rt1me2 = (float)c.rt1me2; r.f.sin_e = (float)c.sin_e;
       r.f.cos_e = (float)c.cos_e; r.f.khat = (float)khat;

@@ -11,6 +11,7 @@
 #include "../../include/pt.h"
 #include "pt_flux.cuh"
 #include "pt_epoch.cuh"
+#include "pt_direct.cuh"
 
 namespace pt {
 
@@ -310,6 +311,16 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
                           (mode == 0 || (size_t)tb->n_z * sizeof(double) <= 110000);
   const bool want_order = n_pv <= kPvCacheMax && n_pv >= 2 &&
                           (want_epoch || plan.mode == 2 || (mode == 1 && plan.mode == 0 && A.n_tiles >= 4 * (int64_t)grid.x * kWarpsPerBlock));
+  // direct kernel: the fp32 variant where there are no epochs to look for (per-row times, or a small problem)
+  if (f32a && n_ss == 1 && !want_epoch) {
+    const bool dv2 = (n_t % 2 == 0) && (t_stride_pv % 2 == 0) && (reinterpret_cast<uintptr_t>(d_times) % 16 == 0) &&
+                     (reinterpret_cast<uintptr_t>(d_flux) % 16 == 0);
+    if (dv2) direct_kernel<2, float, 3><<<grid, kThreads, 0, st>>>(A); else direct_kernel<1, float, 3><<<grid, kThreads, 0, st>>>(A);
+    g_launches.fetch_add(1);
+    const cudaError_t derr = cudaGetLastError();
+    slot_release(ticket, st);
+    return derr == cudaSuccess ? PT_OK : PT_ERR_CUDA;
+  }
   PrepArgs Q{};
   if (want_rec || want_epoch) { Q.rec = slot->pv; Q.n_rec_blocks = (int)((n_pv + kWarpsPerBlock - 1) / kWarpsPerBlock); }
   if (want_axis) { int nb = (int)((n_t + 8 * kThreads - 1) / (8 * kThreads)); Q.n_axis_blocks = nb > 64 ? 64 : nb; }
