@@ -285,6 +285,46 @@ template <class R> static R kepler_E(R M, R e) {
   return (lo + hi) / R(2);
 }
 
+// ---- the other orbit routines the paper names ("circular and elliptic orbits (using either Newton's method,
+// iteration, or two series approximations) ... selects the most appropriate orbit calculation routine based on the
+// eccentricity").  The paper gives no formulas; R19 fixes the reading:
+//   iteration            the fixed-point iteration E <- M + e sin E from E = M (contraction with rate e), run to a fixed point
+//   series, order 3 / 5  the classical expansion of the equation of the centre f - M in powers of e (e.g. Brouwer & Clemence
+//                        1961, ch. II; Murray & Dermott 1999, eq. 2.88), truncated after e^3 and after e^5:
+//     f = M + (2e - e^3/4 + 5e^5/96) sin M + (5e^2/4 - 11e^4/24) sin 2M + (13e^3/12 - 43e^5/64) sin 3M
+//           + (103e^4/96) sin 4M + (1097e^5/960) sin 5M
+//   The position then follows from the true anomaly f: r/a = (1-e^2)/(1 + e cos f).
+enum { SOLVER_EXACT = 0, SOLVER_NEWTON = 1, SOLVER_ITER = 2, SOLVER_PS3 = 3, SOLVER_PS5 = 4, SOLVER_FAST = 5 };
+
+template <class R> static R kepler_E_iteration(R M, R e) {
+  R E = M;
+  for (int it = 0; it < 100000; ++it) {
+    const R En = M + e * x_sin(E);
+    const R d = En > E ? En - E : E - En;
+    E = En;
+    if (d == R(0)) break;                       // a fixed point in this arithmetic
+    const R scale = (E > R(0) ? E : -E) + R(1);
+    if (d <= scale * Real<R>::eps()) break;     // moves by less than an ulp
+  }
+  return E;
+}
+template <class R> static R true_anomaly_series(R M, R e, int order) {
+  const R e2 = e * e, e3 = e2 * e;
+  if (order == 3)
+    return M + (R(2) * e - e3 / R(4)) * x_sin(M) + (R(5) * e2 / R(4)) * x_sin(R(2) * M) + (R(13) * e3 / R(12)) * x_sin(R(3) * M);
+  const R e4 = e2 * e2, e5 = e4 * e;
+  return M + (R(2) * e - e3 / R(4) + R(5) * e5 / R(96)) * x_sin(M) + (R(5) * e2 / R(4) - R(11) * e4 / R(24)) * x_sin(R(2) * M) +
+         (R(13) * e3 / R(12) - R(43) * e5 / R(64)) * x_sin(R(3) * M) + (R(103) * e4 / R(96)) * x_sin(R(4) * M) +
+         (R(1097) * e5 / R(960)) * x_sin(R(5) * M);
+}
+// Which routine the eccentricity selects (R19): exact = circular for e == 0, else a full-precision Kepler
+// solve; fast = the cheapest routine whose truncation error in the true anomaly stays below 2e-9 rad
+// (order 3: 1.5 e^4 <= 2e-9 for e <= 0.006; order 5: 2.2 e^6 <= 2e-9 for e <= 0.03), else the Kepler solve.
+static inline int dispatch_solver(int solver, double e) {
+  if (solver == SOLVER_FAST) return e == 0.0 ? SOLVER_EXACT : (e <= 0.006 ? SOLVER_PS3 : (e <= 0.03 ? SOLVER_PS5 : SOLVER_NEWTON));
+  return solver;
+}
+
 // Projected separation at folded phase ph (cycles, in [-1/2, 1/2]); sign: +z planet in front, -z behind the star.
 // Observer on +Z; t0 is the time of inferior conjunction (true anomaly f = π/2 - w); standard two-body projection.
 template <class R> struct Orbit {
@@ -300,6 +340,31 @@ template <class R> struct Orbit {
     R ftr = Real<R>::pi() / R(2) - R(pr[5]);
     R Etr = R(2) * x_atan2(x_sqrt(R(1) - e) * x_sin(ftr / R(2)), x_sqrt(R(1) + e) * x_cos(ftr / R(2)));
     Mtr = Etr - e * x_sin(Etr);
+  }
+  // `solver`: SOLVER_EXACT / SOLVER_NEWTON = the Kepler solve of this oracle (bisection: "Newton" names the method of the
+  // CUDA path, the root is the same), SOLVER_ITER, SOLVER_PS3, SOLVER_PS5; a non-exact routine is used as asked even for e == 0.
+  R z_signed_solver(double ph, int solver) const {
+    const R pi = Real<R>::pi();
+    if (solver == SOLVER_EXACT || solver == SOLVER_NEWTON) return z_signed(ph);
+    R M = R(2) * pi * R(ph) + Mtr;
+    if (M > pi) M -= R(2) * pi;
+    if (M <= -pi) M += R(2) * pi;
+    R A, B;
+    if (solver == SOLVER_ITER) {
+      R E = kepler_E_iteration<R>(M, e);
+      R cE = x_cos(E), sE = x_sin(E);
+      A = cosw * (cE - e) - sinw * rt1me2 * sE;
+      B = sinw * (cE - e) + cosw * rt1me2 * sE;
+    } else {
+      R f = true_anomaly_series<R>(M, e, solver == SOLVER_PS3 ? 3 : 5);
+      R cf = x_cos(f), sf = x_sin(f);
+      R rr = (R(1) - e) * (R(1) + e) / (R(1) + e * cf);       // r / a
+      A = rr * (cosw * cf - sinw * sf);                       // (r/a) cos(w+f)
+      B = rr * (sinw * cf + cosw * sf);
+    }
+    R Bc = B * cosi;
+    R z = a * x_sqrt(A * A + Bc * Bc);
+    return B > R(0) ? z : -z;
   }
   R z_signed(double ph) const {
     const R pi = Real<R>::pi();
@@ -373,7 +438,7 @@ template <class R> static void interp_basis(const TableView& tb, R khat, R z, R*
 // ---------------------------------------------------------------------------------------------------------
 template <class R>
 static int orbit_z_impl(const double* times, int64_t n_t, int64_t t_stride_pv, const double* params, int64_t n_pv,
-                        int n_pb, int n_ss, double t_exp, double* z_out) {
+                        int n_pb, int n_ss, double t_exp, double* z_out, int solver = SOLVER_EXACT) {
   if (!times || !params || !z_out) return 1;
   if (n_t <= 0 || n_pv <= 0 || n_pb < 1 || n_ss < 1) return 2;
   const int64_t row = 6 + 3 * (int64_t)n_pb;
@@ -387,10 +452,11 @@ static int orbit_z_impl(const double* times, int64_t n_t, int64_t t_stride_pv, c
       continue;
     }
     Orbit<R> orb(pr);
+    const int sv = dispatch_solver(solver, pr[4]);
     for (int64_t j = 0; j < n_t; ++j)
       for (int s = 0; s < n_ss; ++s) {
         double ts = subsample_time(tt[j], t_exp, s, n_ss);
-        zo[j * n_ss + s] = (double)orb.z_signed(fold_phase(ts, pr[0], pr[1]));
+        zo[j * n_ss + s] = (double)orb.z_signed_solver(fold_phase(ts, pr[0], pr[1]), sv);
       }
   }
   return 0;
@@ -509,6 +575,26 @@ int pto_orbit_z(int prec, const double* times, int64_t n_t, int64_t t_stride_pv,
                 int32_t n_pb, int32_t n_ss, double t_exp, double* z_out) {
   return prec == 0 ? orbit_z_impl<double>(times, n_t, t_stride_pv, params, n_pv, n_pb, n_ss, t_exp, z_out)
                    : orbit_z_impl<quad>(times, n_t, t_stride_pv, params, n_pv, n_pb, n_ss, t_exp, z_out);
+}
+
+int pto_orbit_z_solver(int prec, int solver, const double* times, int64_t n_t, int64_t t_stride_pv, const double* params,
+                        int64_t n_pv, int32_t n_pb, int32_t n_ss, double t_exp, double* z_out) {
+  if (solver < SOLVER_EXACT || solver > SOLVER_FAST) return 3;
+  return prec == 0 ? orbit_z_impl<double>(times, n_t, t_stride_pv, params, n_pv, n_pb, n_ss, t_exp, z_out, solver)
+                   : orbit_z_impl<quad>(times, n_t, t_stride_pv, params, n_pv, n_pb, n_ss, t_exp, z_out, solver);
+}
+
+// E(M) by the fixed-point iteration and the true anomaly by the two series, on their own (tests/test_oracle_pins.py).
+int pto_kepler_iter(int prec, const double* M, const double* e, int64_t n, double* E) {
+  for (int64_t i = 0; i < n; ++i)
+    E[i] = prec == 0 ? kepler_E_iteration<double>(M[i], e[i]) : (double)kepler_E_iteration<quad>(quad(M[i]), quad(e[i]));
+  return 0;
+}
+int pto_true_anomaly_series(int prec, int order, const double* M, const double* e, int64_t n, double* f) {
+  if (order != 3 && order != 5) return 3;
+  for (int64_t i = 0; i < n; ++i)
+    f[i] = prec == 0 ? true_anomaly_series<double>(M[i], e[i], order) : (double)true_anomaly_series<quad>(quad(M[i]), quad(e[i]), order);
+  return 0;
 }
 
 int pto_ma_quad_exact(int prec, const double* times, int64_t n_t, int64_t t_stride_pv, const double* params,

@@ -40,7 +40,7 @@ def lib() -> C.CDLL:
     with _lock:
         if _lib is None:
             _lib = C.CDLL(build())
-            for name in ("pto_ma_basis", "pto_ellip", "pto_kepler", "pto_orbit_z", "pto_ma_quad_exact",
+            for name in ("pto_ma_basis", "pto_ellip", "pto_kepler", "pto_kepler_iter", "pto_true_anomaly_series", "pto_orbit_z", "pto_orbit_z_solver", "pto_ma_quad_exact",
                          "pto_ma_table_build", "pto_ma_quad_interp", "pto_interp_basis", "pto_num_threads"):
                 getattr(_lib, name).restype = C.c_int
             _lib.pto_set_num_threads.restype = None
@@ -115,6 +115,41 @@ def orbit_z(times, params, n_pb: int = 1, n_ss: int = 1, t_exp: float = 0.0, pre
                            C.c_int64(n_pv), C.c_int32(n_pb), C.c_int32(n_ss), C.c_double(t_exp), _p(z))
     assert rc == 0, rc
     return z
+
+
+SOLVERS = {"exact": 0, "newton": 1, "iter": 2, "ps3": 3, "ps5": 4, "fast": 5}
+
+
+def orbit_z_solver(times, params, solver: str, n_pb: int = 1, n_ss: int = 1, t_exp: float = 0.0, prec: str = "f128"):
+    """Signed projected separation with one of the orbit routines of P:L31 (R19): 'exact'/'newton' (the Kepler
+    solve), 'iter' (fixed-point iteration), 'ps3'/'ps5' (series of the equation of the centre), 'fast' (e-based dispatch)."""
+    times, params, n_pv, n_t, stride = _shape_args(times, params, n_pb)
+    out = np.empty((n_pv, n_t, n_ss), dtype=np.float64)
+    rc = lib().pto_orbit_z_solver(C.c_int(PREC[prec]), C.c_int(SOLVERS[solver]), _p(times), C.c_int64(n_t), C.c_int64(stride),
+                                  _p(params), C.c_int64(n_pv), C.c_int32(n_pb), C.c_int32(n_ss), C.c_double(t_exp), _p(out))
+    if rc:
+        raise RuntimeError("pto_orbit_z_solver failed: %d" % rc)
+    return out
+
+
+def kepler_iter(M, e, prec: str = "f128"):
+    """E(M) by the fixed-point iteration E <- M + e sin E."""
+    M, e = np.broadcast_arrays(_f64(M), _f64(e))
+    M, e = np.ascontiguousarray(M), np.ascontiguousarray(e)
+    out = np.empty_like(M)
+    lib().pto_kepler_iter(C.c_int(PREC[prec]), _p(M), _p(e), C.c_int64(M.size), _p(out))
+    return out
+
+
+def true_anomaly_series(M, e, order: int, prec: str = "f128"):
+    """True anomaly from the series of the equation of the centre truncated after e^order (order 3 or 5)."""
+    M, e = np.broadcast_arrays(_f64(M), _f64(e))
+    M, e = np.ascontiguousarray(M), np.ascontiguousarray(e)
+    out = np.empty_like(M)
+    rc = lib().pto_true_anomaly_series(C.c_int(PREC[prec]), C.c_int(order), _p(M), _p(e), C.c_int64(M.size), _p(out))
+    if rc:
+        raise RuntimeError("pto_true_anomaly_series failed: %d" % rc)
+    return out
 
 
 def ma_quad_exact(times, params, n_pb: int = 1, n_ss: int = 1, t_exp: float = 0.0, prec: str = "f128"):

@@ -259,6 +259,97 @@ def test_orbit_identities(oracle):
             assert (got > 0) == (mp.sin(mp.mpf(wv[j]) + f) > 0)
 
 
+def _true_anomaly_exact(oracle, M, e):
+    E = oracle.kepler(M, e, "f128")
+    return 2.0 * np.arctan2(np.sqrt(1 + e) * np.sin(E / 2), np.sqrt(1 - e) * np.cos(E / 2))
+
+
+def test_next3_fixed_point_iteration_reaches_the_kepler_root(oracle):
+    # S§8(f) NEXT-3, "iteration": E <- M + e sin E.  Pinned against the bisection solve (a different method) and
+    # against Kepler's equation itself.
+    rng = np.random.default_rng(31)
+    M = rng.uniform(-math.pi, math.pi, 500)
+    e = rng.uniform(0, 0.9, 500)
+    for prec, tol in (("f64", 4e-15), ("f128", 1e-15)):
+        E = oracle.kepler_iter(M, e, prec)
+        assert np.abs(E - e * np.sin(E) - M).max() <= 4 * tol / (1 - 0.9)       # residual / (1 - e cos E) = error in E
+        assert np.abs(E - oracle.kepler(M, e, "f128")).max() <= 4e-14
+    assert np.array_equal(oracle.kepler_iter(M, 0 * e, "f128"), M)               # e -> 0 limit: E = M
+
+
+def test_next3_series_coefficients_are_the_fourier_coefficients_of_the_equation_of_the_centre(oracle):
+    # The two series are truncations of f - M = sum_k c_k(e) sin kM.  The coefficients are pinned against the
+    # mathematics, not against their own formula: c_k(e) = (2/π) ∫_0^π (f - M) sin kM dM of the EXACT true anomaly
+    # (bisection Kepler solve), by the trapezoidal rule on a periodic integrand (spectrally accurate).  A wrong
+    # coefficient (13/12 -> 13/16, a dropped e^5 term, a wrong sign) fails at the e^6 / e^4 level of the remainder.
+    n = 4096
+    M = (np.arange(n) + 0.5) * (2 * math.pi / n) - math.pi
+    for e in (0.02, 0.05, 0.1):
+        ev = np.full(n, e)
+        d_exact = _true_anomaly_exact(oracle, M, ev) - M
+        ck = [(2.0 / n) * np.sum(d_exact * np.sin(k * M)) for k in range(1, 7)]
+        for order, rem in ((3, 3.0 * e ** 4), (5, 4.0 * e ** 6)):
+            d_series = oracle.true_anomaly_series(M, ev, order, "f128") - M
+            sk = [(2.0 / n) * np.sum(d_series * np.sin(k * M)) for k in range(1, 7)]
+            # harmonics the truncation keeps agree up to the first neglected power of e; the ones it drops are absent
+            for k in range(1, 7):
+                assert abs(sk[k - 1] - ck[k - 1]) <= rem + 1e-14, (e, order, k, sk[k - 1], ck[k - 1])
+                if k > order:
+                    assert abs(sk[k - 1]) <= 1e-14
+
+
+def test_next3_series_error_versus_eccentricity_curve(oracle):
+    # error-vs-e curve of the two series against the exact true anomaly: order 3 falls like e^4, order 5 like e^6, and the
+    # constants are those of the first neglected terms; this is what the e-based dispatch of DESIGN.md R19 rests on
+    M = np.linspace(-math.pi, math.pi, 2001)
+    es = np.array([0.003, 0.006, 0.012, 0.03, 0.06, 0.12])
+    err = {3: [], 5: []}
+    for e in es:
+        ev = np.full(M.size, e)
+        fx = _true_anomaly_exact(oracle, M, ev)
+        for order in (3, 5):
+            err[order].append(np.abs(oracle.true_anomaly_series(M, ev, order, "f128") - fx).max())
+    e3, e5 = np.array(err[3]), np.array(err[5])
+    s3 = np.polyfit(np.log(es), np.log(e3), 1)[0]
+    s5 = np.polyfit(np.log(es[2:]), np.log(e5[2:]), 1)[0]          # below e ~ 0.01 the e^6 error sinks under double rounding
+    assert 3.9 <= s3 <= 4.2 and 5.8 <= s5 <= 6.3, (s3, s5)
+    assert np.all(e3 <= 1.5 * es ** 4 * 1.1) and np.all(e3 >= 1.0 * es ** 4)      # max_M |(-11/24) sin 2M + (103/96) sin 4M| = 1.40
+    assert np.all(e5[2:] <= 2.2 * es[2:] ** 6 * 1.2)
+    # the dispatch thresholds: below them the truncation error is under 2e-9 rad
+    assert e3[es <= 0.006].max() <= 2e-9 and e5[es <= 0.03].max() <= 2e-9
+    # e -> 0: every routine tends to the circular orbit
+    rng = np.random.default_rng(32)
+    p = np.array([[0.3, 2.5, 9.0, 1.5, 1e-12, 0.7, 0.1, 0.3, 0.2]])
+    pc = p.copy(); pc[0, 4] = 0.0
+    t = rng.uniform(0, 10, 200)
+    zc = oracle.orbit_z(t, pc, prec="f128")
+    for sv in ("iter", "ps3", "ps5", "fast", "newton"):
+        assert np.abs(np.abs(oracle.orbit_z_solver(t, p, sv, prec="f128")) - np.abs(zc)).max() <= 1e-9
+
+
+def test_next3_orbit_z_by_each_routine(oracle):
+    # z through each routine against the exact orbit: the iteration to rounding, the series within a·|Δf|·(1+e)/(1-e)
+    # (|∂(position)/∂f| <= r_max/a), and the dispatch picks the routine R19 states
+    rng = np.random.default_rng(33)
+    n = 40
+    P, a = rng.uniform(1, 10, n), rng.uniform(3, 20, n)
+    e = np.concatenate([[0.0, 0.004, 0.006, 0.02, 0.03, 0.031], rng.uniform(0, 0.5, n - 6)])
+    pe = np.stack([P * rng.uniform(0, 1, n), P, a, np.arccos(rng.uniform(0, 0.9, n) / a), e, rng.uniform(0, 6.28, n),
+                   0.1 + 0 * P, 0 * P, 0 * P], axis=1)
+    t = np.sort(rng.uniform(0, 30, 400))
+    zx = oracle.orbit_z(t, pe, prec="f128")
+    assert np.abs(oracle.orbit_z_solver(t, pe, "iter", prec="f128") - zx).max() <= 1e-11
+    assert np.array_equal(oracle.orbit_z_solver(t, pe, "newton", prec="f128"), zx)
+    for sv, c, pw in (("ps3", 1.5, 4), ("ps5", 2.2, 6)):
+        dz = np.abs(np.abs(oracle.orbit_z_solver(t, pe, sv, prec="f128")) - np.abs(zx)).max(axis=(1, 2))
+        bound = a * (1 + e) / (1 - e) * c * 1.3 * e ** pw + 1e-12
+        assert np.all(dz <= bound), (sv, (dz / bound).max())
+    zf = oracle.orbit_z_solver(t, pe, "fast", prec="f128")
+    for j in range(n):
+        sv = "exact" if e[j] == 0 else ("ps3" if e[j] <= 0.006 else ("ps5" if e[j] <= 0.03 else "newton"))
+        assert np.array_equal(zf[j], oracle.orbit_z_solver(t, pe[j:j + 1], sv, prec="f128")[0]), (j, e[j])
+
+
 # ------------------------------------------------------------------ supersampling, passbands
 def test_supersampling_is_mean_of_midpoint_subsamples(oracle):
     w = inputs.config2(n_pv=3, n_t=400)
