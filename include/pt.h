@@ -78,6 +78,22 @@ int pt_build_arch(void);
 int pt_orbit_z(const double* d_times, int64_t n_t, int64_t t_stride_pv, const double* d_params, int64_t n_pv,
                int32_t n_pb, int32_t n_ss, double t_exp, double* d_z, void* stream);
 
+/* The other orbit routines the paper names ("circular and elliptic orbits (using either Newton's method, iteration,
+ * or two series approximations) ... selects the most appropriate orbit calculation routine based on the eccentricity";
+ * SURVEY §8(f) NEXT-3).  The paper prints no formulas; R19 fixes the reading:
+ *   PT_SOLVER_EXACT   e == 0: circular routine, else Newton on Kepler's equation (what pt_orbit_z and every flux entry use)
+ *   PT_SOLVER_NEWTON  the same
+ *   PT_SOLVER_ITER    fixed-point iteration E <- M + e sin E from E = M, run until E moves by less than an ulp
+ *   PT_SOLVER_PS3/5   true anomaly from the classical series of the equation of the centre f - M in powers of e, truncated
+ *                     after e^3 / e^5; truncation error in f at most 1.5 e^4 / 2.2 e^6 rad, in z at most a (1+e)/(1-e)
+ *                     times that
+ *   PT_SOLVER_FAST    by eccentricity: e == 0 circular, e <= 0.006 order 3, e <= 0.03 order 5 (truncation error below
+ *                     2e-9 rad in f), else Newton
+ * Same arguments, layout and error behaviour as pt_orbit_z; an unknown solver is PT_ERR_SIZE. */
+enum { PT_SOLVER_EXACT = 0, PT_SOLVER_NEWTON = 1, PT_SOLVER_ITER = 2, PT_SOLVER_PS3 = 3, PT_SOLVER_PS5 = 4, PT_SOLVER_FAST = 5 };
+int pt_orbit_z_solver(const double* d_times, int64_t n_t, int64_t t_stride_pv, const double* d_params, int64_t n_pv,
+                      int32_t n_pb, int32_t n_ss, double t_exp, int32_t solver, double* d_z, void* stream);
+
 /* S0-S7: exact quadratic Mandel–Agol flux (Eq. 13 with P:L143).
  *   dtype  PT_F64: d_flux is double.  PT_F32 / PT_F32S: d_flux is float (see the enum above).
  *   d_flux [n_pv][n_pb][n_t], time fastest.   d_status: NULL or 2 x int32 (see above). */

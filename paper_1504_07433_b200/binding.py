@@ -20,7 +20,7 @@ PT_F64, PT_F32, PT_F32S = 0, 1, 2
 PT_ST_BAD_PARAM, PT_ST_K_OUT_OF_TABLE = 1, 2
 _ERR = {1: "PT_ERR_NULL", 2: "PT_ERR_SIZE", 3: "PT_ERR_DTYPE", 4: "PT_ERR_TABLE", 5: "PT_ERR_CUDA"}
 
-EXPORTS = ("pt_build_arch", "pt_orbit_z", "pt_ma_quad_exact", "pt_ma_table_build", "pt_table_spacing", "pt_ma_quad_interp", "pt_ma_quad_chi2", "pt_ma_quad_exact_pbk",
+EXPORTS = ("pt_build_arch", "pt_orbit_z", "pt_orbit_z_solver", "pt_ma_quad_exact", "pt_ma_table_build", "pt_table_spacing", "pt_ma_quad_interp", "pt_ma_quad_chi2", "pt_ma_quad_exact_pbk",
            "pt_ma_quad_exact_host", "pt_ma_quad_interp_host", "pt_plan", "pt_probe_dfma", "pt_launch_count")
 
 
@@ -49,6 +49,7 @@ def lib() -> C.CDLL:
         L.pt_build_arch.restype = C.c_int
         L.pt_launch_count.restype = i64
         L.pt_orbit_z.argtypes = common + [ptr, ptr]
+        L.pt_orbit_z_solver.argtypes = common + [i32, ptr, ptr]
         L.pt_ma_quad_exact.argtypes = common + [i32, ptr, ptr, ptr]
         L.pt_ma_quad_exact_pbk.argtypes = common + [i32, ptr, ptr, ptr]
         L.pt_ma_table_build.argtypes = [dbl, dbl, i32, dbl, i32, i32, i32, ptr, ptr]
@@ -113,6 +114,22 @@ def pt_orbit_z(times: torch.Tensor, params: torch.Tensor, n_pb: int = 1, n_ss: i
         out = torch.empty((n_pv, n_t, n_ss), dtype=torch.float64, device=times.device)
     _check(lib().pt_orbit_z(times.data_ptr(), n_t, stride, params.data_ptr(), n_pv, n_pb, n_ss, float(t_exp),
                             out.data_ptr(), _stream()), "pt_orbit_z")
+    return out
+
+
+SOLVERS = {"exact": 0, "newton": 1, "iter": 2, "ps3": 3, "ps5": 4, "fast": 5}
+
+
+def pt_orbit_z_solver(times: torch.Tensor, params: torch.Tensor, solver: str, n_pb: int = 1, n_ss: int = 1,
+                      t_exp: float = 0.0, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """Signed projected separation by one of the orbit routines of P:L31 (include/pt.h: pt_orbit_z_solver)."""
+    times, params, n_pv, n_t, stride = _marshal(times, params, n_pb)
+    if solver not in SOLVERS:
+        raise PtError("solver must be one of %s" % sorted(SOLVERS))
+    if out is None:
+        out = torch.empty((n_pv, n_t, n_ss), dtype=torch.float64, device=times.device)
+    _check(lib().pt_orbit_z_solver(times.data_ptr(), n_t, stride, params.data_ptr(), n_pv, n_pb, n_ss, float(t_exp),
+                                   SOLVERS[solver], out.data_ptr(), _stream()), "pt_orbit_z_solver")
     return out
 
 

@@ -112,8 +112,10 @@ static void slot_release(const SlotTicket& t, cudaStream_t st) {
 __global__ void __launch_bounds__(kThreads) orbit_kernel(const double* __restrict__ times, int64_t n_t,
                                                          int64_t t_stride_pv, const double* __restrict__ params,
                                                          int n_pb, int n_ss, double t_exp, double* __restrict__ z_out,
-                                                         int blocks_per_pv) {
+                                                         int blocks_per_pv, int solver) {
   __shared__ PvConst c;
+  __shared__ double ser[5];
+  __shared__ int s_solver;
   const int64_t pv = blockIdx.x / blocks_per_pv;
   const int chunk = (int)(blockIdx.x % blocks_per_pv);
   const double* row = params + pv * (6 + 3 * (int64_t)n_pb);
@@ -127,8 +129,24 @@ __global__ void __launch_bounds__(kThreads) orbit_kernel(const double* __restric
     }
     c.khat = ksum / (double)n_pb;
     pv_setup_orbit(c, row, ok, n_ss, t_exp);
+    // the routine for this parameter vector ("selects the most appropriate orbit calculation routine based on the
+    // eccentricity"); a non-exact routine asked for by name is used even for e == 0 (w and Mtr are then set up as for e > 0)
+    int sv = (c.flags & PV_BAD) ? SOLVER_EXACT : dispatch_solver(solver, c.e);
+    if (sv == SOLVER_NEWTON) sv = SOLVER_EXACT;
+    if (sv != SOLVER_EXACT) {
+      if (c.flags & PV_CIRCULAR) {   // e == 0 through an eccentric routine: conjunction at true anomaly π/2 - w
+        double w = row[5];
+        sincos(w, &c.sinw, &c.cosw);
+        c.rt1me2 = 1.0;
+        const double ftr = 0.5 * kPi - atan2(c.sinw, c.cosw);
+        c.Mtr = ftr - kTwoPi * rint(ftr * (1.0 / kTwoPi));
+      }
+      series_coefficients(c.e, sv == SOLVER_PS3 ? 3 : 5, ser);
+    }
+    s_solver = sv;
   }
   __syncthreads();
+  const int sv = s_solver;
   const int64_t n = n_t * n_ss;
   const double* tt = times + pv * t_stride_pv;
   double* zo = z_out + pv * n;
@@ -141,7 +159,8 @@ __global__ void __launch_bounds__(kThreads) orbit_kernel(const double* __restric
       const int s = (int)(i - e * n_ss);
       const double t = __ldg(tt + e);
       const double ts = (n_ss > 1) ? __dadd_rn(t, subsample_offset(s, n_ss, t_exp)) : t;
-      z = orbit_z_signed(c, fold_phase(ts, c.t0, c.P, c.invP, c.flags & PV_SLOWDIV));
+      const double ph = fold_phase(ts, c.t0, c.P, c.invP, c.flags & PV_SLOWDIV);
+      z = (sv == SOLVER_EXACT) ? orbit_z_signed(c, ph) : orbit_z_signed_alt(c, ser, ph, sv);
     }
     zo[i] = z;
   }
@@ -461,8 +480,14 @@ int pt_probe_dfma(int32_t blocks, int32_t iters, double* d_sink, void* stream) {
 
 int pt_orbit_z(const double* d_times, int64_t n_t, int64_t t_stride_pv, const double* d_params, int64_t n_pv,
                int32_t n_pb, int32_t n_ss, double t_exp, double* d_z, void* stream) {
+  return pt_orbit_z_solver(d_times, n_t, t_stride_pv, d_params, n_pv, n_pb, n_ss, t_exp, PT_SOLVER_EXACT, d_z, stream);
+}
+
+int pt_orbit_z_solver(const double* d_times, int64_t n_t, int64_t t_stride_pv, const double* d_params, int64_t n_pv,
+                      int32_t n_pb, int32_t n_ss, double t_exp, int32_t solver, double* d_z, void* stream) {
   int rc = check_common(d_times, d_params, d_z, n_t, t_stride_pv, n_pv, n_pb, n_ss);
   if (rc) return rc;
+  if (solver < PT_SOLVER_EXACT || solver > PT_SOLVER_FAST) return PT_ERR_SIZE;
   const int64_t n = n_t * n_ss;
   int64_t bpp = (n + (int64_t)kThreads * 8 - 1) / ((int64_t)kThreads * 8);
   const int64_t cap = ((int64_t)sm_count() * 16 + n_pv - 1) / n_pv;
@@ -470,7 +495,7 @@ int pt_orbit_z(const double* d_times, int64_t n_t, int64_t t_stride_pv, const do
   if (bpp < 1) bpp = 1;
   if (n_pv * bpp > 0x7fffffff) return PT_ERR_SIZE;
   orbit_kernel<<<(unsigned)(n_pv * bpp), kThreads, 0, (cudaStream_t)stream>>>(d_times, n_t, t_stride_pv, d_params, n_pb,
-                                                                              n_ss, t_exp, d_z, (int)bpp);
+                                                                              n_ss, t_exp, d_z, (int)bpp, (int)solver);
   g_launches.fetch_add(1);
   return cudaGetLastError() == cudaSuccess ? PT_OK : PT_ERR_CUDA;
 }

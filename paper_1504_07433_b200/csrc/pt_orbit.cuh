@@ -143,6 +143,72 @@ __device__ __forceinline__ double orbit_z_signed(const PvConst& c, double ph) {
   return B > 0.0 ? z : -z;
 }
 
+// ---- the other orbit routines of P:L31 (R19): fixed-point iteration and the two series
+// approximations of the equation of the centre, selectable per call (pt_orbit_z_solver) or by the eccentricity.
+enum OrbitSolver : int { SOLVER_EXACT = 0, SOLVER_NEWTON = 1, SOLVER_ITER = 2, SOLVER_PS3 = 3, SOLVER_PS5 = 4, SOLVER_FAST = 5 };
+
+// The routine the eccentricity selects: exact = circular for e == 0 else Newton; fast = the cheapest routine whose
+// truncation error in the true anomaly is below 2e-9 rad (order 3: 1.5 e^4, e <= 0.006; order 5: 2.2 e^6, e <= 0.03).
+__host__ __device__ __forceinline__ int dispatch_solver(int solver, double e) {
+  if (solver == SOLVER_FAST) return e == 0.0 ? SOLVER_EXACT : (e <= 0.006 ? SOLVER_PS3 : (e <= 0.03 ? SOLVER_PS5 : SOLVER_NEWTON));
+  return solver;
+}
+
+// Coefficients of sin kM, k = 1..5, of f - M truncated after e^3 (order 3) or e^5 (classical expansion, e.g. Murray &
+// Dermott 1999 eq. 2.88): once per parameter vector.
+__device__ __forceinline__ void series_coefficients(double e, int order, double* c) {
+  const double e2 = e * e, e3 = e2 * e;
+  if (order == 3) {
+    c[0] = 2.0 * e - 0.25 * e3; c[1] = 1.25 * e2; c[2] = (13.0 / 12.0) * e3; c[3] = 0.0; c[4] = 0.0;
+  } else {
+    const double e4 = e2 * e2, e5 = e4 * e;
+    c[0] = 2.0 * e - 0.25 * e3 + (5.0 / 96.0) * e5;
+    c[1] = 1.25 * e2 - (11.0 / 24.0) * e4;
+    c[2] = (13.0 / 12.0) * e3 - (43.0 / 64.0) * e5;
+    c[3] = (103.0 / 96.0) * e4;
+    c[4] = (1097.0 / 960.0) * e5;
+  }
+}
+
+// Signed projected separation by one of the non-default routines: SOLVER_ITER (E <- M + e sin E from E = M until it moves
+// by less than an ulp; linear convergence with rate e) or SOLVER_PS3 / SOLVER_PS5 (series for the true anomaly, `ser` from
+// series_coefficients; sin kM by the Chebyshev recurrence from one sincos).
+__device__ __forceinline__ double orbit_z_signed_alt(const PvConst& c, const double* ser, double ph, int solver) {
+  double M = fma(kC[C_TWOPI], ph, c.Mtr);
+  if (M > kC[C_PI]) M -= kC[C_TWOPI];
+  if (M <= -kC[C_PI]) M += kC[C_TWOPI];
+  double A, B;
+  if (solver == SOLVER_ITER) {
+    double E = M, sE, cE;
+#pragma unroll 1
+    for (int it = 0; it < 100000; ++it) {
+      sincos_bounded(E, &sE, &cE);
+      const double En = fma(c.e, sE, M);
+      const double d = fabs(En - E);
+      E = En;
+      if (d <= 0x1p-53 * (fabs(E) + 1.0)) break;
+    }
+    sincos_bounded(E, &sE, &cE);
+    const double x = cE - c.e, y = c.rt1me2 * sE;
+    A = c.cosw * x - c.sinw * y;
+    B = c.sinw * x + c.cosw * y;
+  } else {
+    double s1, c1;
+    sincos_bounded(M, &s1, &c1);
+    const double tc = 2.0 * c1;
+    const double s2 = tc * s1, s3 = fma(tc, s2, -s1), s4 = fma(tc, s3, -s2), s5 = fma(tc, s4, -s3);
+    const double f = M + fma(ser[4], s5, fma(ser[3], s4, fma(ser[2], s3, fma(ser[1], s2, ser[0] * s1))));
+    double sf, cf;
+    sincos_bounded(f, &sf, &cf);
+    const double rr = (1.0 - c.e) * (1.0 + c.e) * rcp_fast(fma(c.e, cf, 1.0));   // r / a
+    A = rr * (c.cosw * cf - c.sinw * sf);
+    B = rr * (c.sinw * cf + c.cosw * sf);
+  }
+  const double Bc = B * c.cosi;
+  const double z = c.a * sqrt_fast(fmax(fma(A, A, Bc * Bc), 0x1p-1000));
+  return B > 0.0 ? z : -z;
+}
+
 // Mean anomaly of true anomaly f (|f| up to a few turns), reduced to (-π, π]: tan(E/2) = sqrt((1-e)/(1+e)) tan(f/2),
 // M = E - e sin E.  rm = sqrt(1-e), rp = sqrt(1+e).  Lean primitives (pt_math.cuh): this runs once per tile.
 __device__ __forceinline__ double mean_anomaly_of_true(double f, double e, double rm, double rp) {

@@ -110,6 +110,55 @@ def test_high_eccentricity_and_long_baseline(pt, oracle):
     assert np.abs(z - zr).max() <= 1e-11
 
 
+# ------------------------------------------------------------------------------------------- NEXT-3: the other orbit routines
+@pytest.mark.parametrize("solver", ["newton", "iter", "ps3", "ps5", "fast"])
+def test_orbit_solvers_parity(pt, oracle, solver):
+    # Each routine of P:L31 against the SAME routine of the oracle in __float128 (R19).  Both sides evaluate the
+    # same mathematical function (the root of Kepler's equation, or the same truncated series), so the tolerance is the
+    # rounding of the fp64 evaluation: |Δz| <= a (1+e)/(1-e) x (a few ulp of the anomaly) — 1e-11 covers a <= 30, e <= 0.6;
+    # the iteration stops when E moves by less than an ulp, i.e. within e/(1-e) ulp of its fixed point.
+    rng = np.random.default_rng(41)
+    n = 96
+    P, a = rng.uniform(1, 10, n), rng.uniform(3, 30, n)
+    emax = 0.6 if solver in ("newton", "iter", "fast") else 0.2
+    e = rng.uniform(0, emax, n)
+    e[:8] = [0.0, 1e-9, 0.004, 0.006, 0.0061, 0.03, 0.0301, 0.1]
+    pe = np.stack([P * rng.uniform(0, 1, n), P, a, np.arccos(rng.uniform(0, 0.95, n) / a), e, rng.uniform(0, 2 * math.pi, n),
+                   rng.uniform(0.02, 0.3, n), 0.3 + 0 * P, 0.2 + 0 * P], axis=1)
+    pe[40, 1] = -1.0                                       # a bad row stays NaN whatever the routine
+    t = np.sort(rng.uniform(0, 100, 1500))
+    z = pt.pt_orbit_z_solver(dev(t), dev(pe), solver).cpu().numpy()
+    zr = oracle.orbit_z_solver(t, pe, solver, prec="f128")
+    assert np.array_equal(np.isnan(z), np.isnan(zr)) and np.all(np.isnan(z[40]))
+    ok = ~np.isnan(zr)
+    assert np.abs(z[ok] - zr[ok]).max() <= 1e-11
+    # supersampled and per-row times through the same entry point
+    tt = np.sort(rng.uniform(0, 50, (n, 64)), axis=1)
+    z2 = pt.pt_orbit_z_solver(dev(tt), dev(pe), solver, 1, 3, 0.02).cpu().numpy()
+    zr2 = oracle.orbit_z_solver(tt, pe, solver, 1, 3, 0.02, prec="f128")
+    ok = ~np.isnan(zr2)
+    assert np.abs(z2[ok] - zr2[ok]).max() <= 1e-11
+    if solver in ("newton", "fast"):
+        # exact routines: also the plain entry point; the dispatch picks the series only where its error is below 2e-9 rad
+        zx = pt.pt_orbit_z(dev(t), dev(pe)).cpu().numpy()
+        okx = ~np.isnan(zx)
+        bound = (a * (1 + e) / (1 - e) * 2.1e-9)[:, None, None] + 1e-11
+        assert np.all((np.abs(np.abs(z) - np.abs(zx)) <= bound)[okx])
+        if solver == "newton":
+            assert np.array_equal(z[okx], zx[okx])
+
+
+def test_orbit_solver_argument_errors(pt):
+    from paper_1504_07433_b200 import binding
+    t = torch.zeros(8, dtype=torch.float64, device="cuda")
+    p = torch.zeros((1, 9), dtype=torch.float64, device="cuda")
+    o = torch.zeros(8, dtype=torch.float64, device="cuda")
+    L = binding.lib()
+    assert L.pt_orbit_z_solver(t.data_ptr(), 8, 0, p.data_ptr(), 1, 1, 1, 0.0, 6, o.data_ptr(), None) == binding.PT_ERR_SIZE
+    assert L.pt_orbit_z_solver(t.data_ptr(), 8, 0, p.data_ptr(), 1, 1, 1, 0.0, -1, o.data_ptr(), None) == binding.PT_ERR_SIZE
+    assert L.pt_orbit_z_solver(None, 8, 0, p.data_ptr(), 1, 1, 1, 0.0, 2, o.data_ptr(), None) == binding.PT_ERR_NULL
+
+
 # ------------------------------------------------------------------------------------------- degenerate inputs
 def test_edge_cases_k_and_geometry(pt, oracle):
     t = np.linspace(-0.3, 0.3, 1501)
