@@ -163,6 +163,8 @@ int pt_ma_quad_interp_host(const pt_table* table, const double* h_times, int64_t
  * every thread of `blocks` x 256 runs `iters` rounds of 8 independent DFMA chains and stores one double to
  * d_sink[blocks*256] so the work cannot be removed.  FP64 thread-instructions issued = blocks*256*iters*8. */
 int pt_probe_dfma(int32_t blocks, int32_t iters, double* d_sink, void* stream);
+/* The same for the FP32 pipe (roofline denominator of the fp32 variant): FFMA chains, d_sink: blocks*256 floats. */
+int pt_probe_ffma(int32_t blocks, int32_t iters, float* d_sink, void* stream);
 
 /* How the flux kernels would cut up a problem on a device with n_sm multiprocessors (pure host logic, no CUDA call; used
  * by the CPU tests).  h_out[0] = exposures per tile, [1] = tiles per parameter vector, [2] = scheduling mode (0 global

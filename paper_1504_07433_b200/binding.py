@@ -21,7 +21,7 @@ PT_ST_BAD_PARAM, PT_ST_K_OUT_OF_TABLE = 1, 2
 _ERR = {1: "PT_ERR_NULL", 2: "PT_ERR_SIZE", 3: "PT_ERR_DTYPE", 4: "PT_ERR_TABLE", 5: "PT_ERR_CUDA"}
 
 EXPORTS = ("pt_build_arch", "pt_orbit_z", "pt_orbit_z_solver", "pt_ma_quad_exact", "pt_ma_table_build", "pt_table_spacing", "pt_ma_quad_interp", "pt_ma_quad_chi2", "pt_ma_quad_exact_pbk",
-           "pt_ma_quad_exact_host", "pt_ma_quad_interp_host", "pt_plan", "pt_probe_dfma", "pt_launch_count")
+           "pt_ma_quad_exact_host", "pt_ma_quad_interp_host", "pt_plan", "pt_probe_dfma", "pt_probe_ffma", "pt_launch_count")
 
 
 class PtError(RuntimeError):
@@ -59,6 +59,7 @@ def lib() -> C.CDLL:
         L.pt_ma_quad_exact_host.argtypes = common + [i32, ptr, ptr]
         L.pt_ma_quad_interp_host.argtypes = [C.POINTER(pt_table)] + common + [i32, ptr, ptr]
         L.pt_probe_dfma.argtypes = [i32, i32, ptr, ptr]
+        L.pt_probe_ffma.argtypes = [i32, i32, ptr, ptr]
         L.pt_plan.argtypes = [i64, i64, i32, C.POINTER(C.c_int64)]
         for n in EXPORTS[1:-1]:
             getattr(L, n).restype = C.c_int
@@ -234,6 +235,13 @@ def pt_ma_quad_interp_host(table: Table, times: torch.Tensor, params: torch.Tens
                                         n_pb, n_ss, float(t_exp), _dtype_code(out.dtype), out.data_ptr(),
                                         status.data_ptr() if status is not None else None), "pt_ma_quad_interp_host")
     return out
+
+
+def pt_probe_ffma(blocks: int, iters: int, sink: torch.Tensor) -> None:
+    """FP32-pipe peak probe (include/pt.h: pt_probe_ffma); sink: CUDA float32 tensor of blocks*256 elements."""
+    if not sink.is_cuda or sink.dtype != torch.float32 or sink.numel() < blocks * 256:
+        raise PtError("sink must be a CUDA float32 tensor of at least blocks*256 elements")
+    _check(lib().pt_probe_ffma(blocks, iters, sink.data_ptr(), _stream()), "pt_probe_ffma")
 
 
 def pt_probe_dfma(blocks: int, iters: int, sink: torch.Tensor) -> None:

@@ -198,6 +198,18 @@ __global__ void __launch_bounds__(kThreads) dfma_probe_kernel(int iters, double*
   sink[(size_t)blockIdx.x * kThreads + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
 }
 
+// FP32-pipe peak probe: 8 independent FFMA chains per thread.
+__global__ void __launch_bounds__(kThreads) ffma_probe_kernel(int iters, float* __restrict__ sink) {
+  float a0 = threadIdx.x * 1e-3f, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+  const float m = 0.999999f, c = 1e-6f;
+#pragma unroll 4
+  for (int i = 0; i < iters; ++i) {
+    a0 = fmaf(a0, m, c); a1 = fmaf(a1, m, c); a2 = fmaf(a2, m, c); a3 = fmaf(a3, m, c);
+    a4 = fmaf(a4, m, c); a5 = fmaf(a5, m, c); a6 = fmaf(a6, m, c); a7 = fmaf(a7, m, c);
+  }
+  sink[(size_t)blockIdx.x * kThreads + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+}
+
 // ------------------------------------------------------------------------------------------------ host side
 static int check_common(const void* times, const void* params, const void* out, int64_t n_t, int64_t t_stride_pv,
                         int64_t n_pv, int n_pb, int n_ss) {
@@ -475,6 +487,13 @@ int pt_probe_dfma(int32_t blocks, int32_t iters, double* d_sink, void* stream) {
   if (!d_sink) return PT_ERR_NULL;
   if (blocks < 1 || iters < 1) return PT_ERR_SIZE;
   dfma_probe_kernel<<<(unsigned)blocks, kThreads, 0, (cudaStream_t)stream>>>(iters, d_sink);
+  return cudaGetLastError() == cudaSuccess ? PT_OK : PT_ERR_CUDA;
+}
+
+int pt_probe_ffma(int32_t blocks, int32_t iters, float* d_sink, void* stream) {
+  if (!d_sink) return PT_ERR_NULL;
+  if (blocks < 1 || iters < 1) return PT_ERR_SIZE;
+  ffma_probe_kernel<<<(unsigned)blocks, kThreads, 0, (cudaStream_t)stream>>>(iters, d_sink);
   return cudaGetLastError() == cudaSuccess ? PT_OK : PT_ERR_CUDA;
 }
 

@@ -179,14 +179,16 @@ __device__ __forceinline__ double orbit_z_signed_alt(const PvConst& c, const dou
   if (M <= -kC[C_PI]) M += kC[C_TWOPI];
   double A, B;
   if (solver == SOLVER_ITER) {
-    double E = M, sE, cE;
+    double E = M, sE, cE, dprev = CUDART_INF;
 #pragma unroll 1
     for (int it = 0; it < 100000; ++it) {
       sincos_bounded(E, &sE, &cE);
       const double En = fma(c.e, sE, M);
       const double d = fabs(En - E);
       E = En;
-      if (d <= 0x1p-53 * (fabs(E) + 1.0)) break;
+      // a fixed point to rounding: the step is below an ulp, or it no longer shrinks (the last bit may flip for ever)
+      if (d <= 0x1p-53 * (fabs(E) + 1.0) || (d >= dprev && d <= 0x1p-48 * (fabs(E) + 1.0))) break;
+      dprev = d;
     }
     sincos_bounded(E, &sE, &cE);
     const double x = cE - c.e, y = c.rt1me2 * sE;
