@@ -265,6 +265,12 @@ static Plan plan_tiles(int64_t n_pv, int64_t n_t, int n_sm) {
   tl = (tl + 255) / 256 * 256;
   if (tl < 256) tl = 256;
   if (tl > 16384) tl = 16384;
+  if (total < (double)(64 * n_sm)) {
+    // a tiny problem (configs[0]: 1000 exposures) is a latency, not a throughput: short tiles, so that it is one round of
+    // many warps instead of many rounds of a few
+    tl = ((int64_t)(total / (double)(2 * n_sm)) + 31) / 32 * 32;
+    tl = tl < 32 ? 32 : (tl > 256 ? 256 : tl);
+  }
   int64_t tpp = (n_t + tl - 1) / tl;
   const bool few = (n_pv <= kSchedWords - kSchedHead - kBaseBlocks && tpp >= 2);   // the slot's tail holds the chi2 partials
   p.mode = few ? 1 : 0;
@@ -334,7 +340,8 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   //   axis     one shared time axis of a problem large enough for the extra launch to pay: is it ascending?
   //   order    global tile counter: heaviest rows first (mode 2), or rows by k̂ for the interpolated model
   //   baseline fused likelihood
-  const bool want_rec = n_pb == 1 && pb_view < 0 && n_pv <= kPvCacheMax && A.n_tiles >= 8 * n_pv;
+  const bool want_rec = n_pb == 1 && pb_view < 0 && n_pv <= kPvCacheMax && A.n_tiles >= 8 * n_pv &&
+                        (double)n_pv * (double)n_t >= 65536.0;   // a small problem does not pay for the extra launch
   const bool want_axis = t_stride_pv == 0 && n_t >= 2048 && (double)n_pv * (double)n_t >= (double)PT_RANGE_MIN;
   // epoch kernel: one passband on one shared axis that prep_kernel checks; it does the whole launch if the axis is ascending,
   // else the general kernel launched behind it does

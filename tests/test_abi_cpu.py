@@ -109,9 +109,9 @@ def test_launch_plan_host_logic(libpath):
     p = binding.pt_plan(64, 60000)
     assert p["mode"] == 2 and p["tile_len"] % 256 == 0 and p["blocks"] == 148 * 3
     assert p["tiles_per_pv"] == -(-60000 // p["tile_len"]) and 64 * p["tiles_per_pv"] >= 2 * warps
-    # configs[0]: one short row -> one block is enough, a global counter
+    # configs[0]: one short row -> a latency: short tiles, one round of many warps
     p = binding.pt_plan(1, 1000)
-    assert p["mode"] in (0, 1) and p["blocks"] == 1 and p["tile_len"] * p["tiles_per_pv"] >= 1000
+    assert p["mode"] in (0, 1) and p["tile_len"] == 32 and p["blocks"] == 4 and p["tile_len"] * p["tiles_per_pv"] >= 1000
     # configs[2]: 512 rows of 600 -> fewer tiles than warps: no ranking, per-row counters
     p = binding.pt_plan(512, 600)
     assert p["mode"] == 1 and p["tiles_per_pv"] == 3
@@ -125,7 +125,8 @@ def test_launch_plan_host_logic(libpath):
     for n_pv, n_t, n_sm in ((1, 1, 148), (3, 255, 148), (3, 257, 132), (1000, 7, 148), (7, 10 ** 7, 148), (10 ** 6, 3, 148),
                             (448, 60000, 148), (2, 2 ** 31 - 1, 8)):
         p = binding.pt_plan(n_pv, n_t, n_sm)
-        assert 256 <= p["tile_len"] <= 16384 and p["tile_len"] % 256 == 0
+        assert 32 <= p["tile_len"] <= 16384 and p["tile_len"] % 32 == 0
+        assert p["tile_len"] % 256 == 0 or n_pv * n_t < 64 * n_sm              # short tiles only for tiny problems
         assert (p["tiles_per_pv"] - 1) * p["tile_len"] < n_t <= p["tiles_per_pv"] * p["tile_len"]
         assert 1 <= p["blocks"] <= n_sm * 3
     with pytest.raises(binding.PtError):

@@ -599,6 +599,36 @@ def test_range_mode_axis_variants(pt, oracle, axis, n_ss):
         assert np.abs(c - rc).max() <= 1e-10 * np.abs(rc).max()
 
 
+@pytest.mark.parametrize("n_pv,n_t,n_ss", [(64, 4097, 10), (17, 2500, 1), (40, 6001, 3), (40, 6000, 40), (300, 2048, 1)])
+def test_epoch_kernel_writes_every_element(pt, oracle, n_pv, n_t, n_ss):
+    """The epoch kernel (one passband, shared ascending axis) partitions every row into gaps (pure fills) and transit
+    windows (evaluated) found by search: an output buffer pre-filled with NaN must come back without one, for the exact
+    and the interpolated model, fp64 and fp32 flux, even and odd row lengths, rows that never transit, rows cut into
+    chunks (short periods, planet always overlapping) and bad rows."""
+    w = inputs.config2(n_pv=n_pv, n_t=n_t)
+    w.n_ss = n_ss
+    p = w.params
+    p[0, 1] = 0.05; p[1, 1] = 0.11; p[2, 2] = 1.05; p[3, 3] = 0.3; p[5, 6] = 0.0; p[6, 1] = 5000.0; p[7, 0] = 1e6
+    p[4, 1] = -1.0                                           # bad row: NaN on both sides
+    t, dp = dev(w.times), dev(p)
+    r = ora_exact(oracle, w)
+    for dtype, tol in ((torch.float64, TOL64), (torch.float32, TOL32)):
+        out = torch.full((n_pv, 1, n_t), float("nan"), dtype=dtype, device="cuda")
+        pt.pt_ma_quad_exact(t, dp, 1, w.n_ss, w.t_exp, out=out)
+        f = out.cpu().numpy().astype(np.float64)
+        assert np.array_equal(np.isnan(f), np.isnan(r)) and np.all(np.isnan(f[4]))
+        ok = ~np.isnan(r)
+        assert np.abs(f[ok] - r[ok]).max() <= tol
+    tb = pt.pt_ma_table_build(dtype=torch.float32, n_fn=4, k_min=0.05, k_max=0.25, n_k=41, z_max=1.25, n_z=1251)
+    out = torch.full((n_pv, 1, n_t), float("nan"), dtype=torch.float64, device="cuda")
+    pt.pt_ma_quad_interp(tb, t, dp, 1, w.n_ss, w.t_exp, out=out)
+    ri = oracle.ma_quad_interp(tb.data.cpu().numpy(), tb.k_min, tb.dk, tb.dz, w.times, p, 1, w.n_ss, w.t_exp, prec="f128")
+    f = out.cpu().numpy()
+    assert np.array_equal(np.isnan(f), np.isnan(ri))
+    ok = ~np.isnan(ri)
+    assert np.abs(f[ok] - ri[ok]).max() <= TOL64
+
+
 def test_range_mode_multipassband_and_fp32(pt, oracle):
     rng = np.random.default_rng(5)
     n_pv, n_pb, n_t = 40, 3, 6000
