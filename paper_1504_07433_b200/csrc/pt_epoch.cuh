@@ -271,6 +271,7 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? 24 : 2)) epoch_kernel(const __
         if (lane == 0) phi = phi0;
         for (int i = 0; i < m; ++i) {
           const int a = __shfl_sync(0xffffffffu, phi, i), b = __shfl_sync(0xffffffffu, lo, i);
+          PT_CHECK(a >= 0 && b <= n_t);                      // a > b never happens (the windows are disjoint) and would be a no-op
           if constexpr (!kIsChi2<OutT>) fill_span<V2, OutT>(row, (uint32_t)a, (uint32_t)b, (OutT)1.0);
         }
         if constexpr (!kIsChi2<OutT>) {
@@ -319,6 +320,7 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? 24 : 2)) epoch_kernel(const __
             const int x = q * 32 + lane;
             act = x < n_exp;
             e = exposure_of(act ? x : n_exp - 1);
+            PT_CHECK(e >= 0 && e < n_t);
             t = act ? ldg_keep(A.times + e, pol) : 0.0;
             if constexpr (kIsChi2<OutT>) {     // the observation this exposure will be compared with: towards L1 now
               if (act) {
@@ -348,6 +350,7 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? 24 : 2)) epoch_kernel(const __
             const int x = x0 + dx, sub = v - dx * n_ss;
             const bool act = x < n_exp;
             const int e = exposure_of(act ? x : n_exp - 1);
+            PT_CHECK(e >= 0 && e < n_t && sub >= 0 && sub < n_ss);
             long long fx = 0;
             if (act) {
               const double t = ldg_keep(A.times + e, pol);
@@ -365,6 +368,7 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? 24 : 2)) epoch_kernel(const __
             const int snext = __shfl_down_sync(0xffffffffu, sid, 1);
             if (act && (lane == 31 || snext != sid)) {       // last subsample of this exposure in this round
               const long long sum = W.acc[x & (kAccRing - 1)] + fx;
+              PT_CHECK(sub == n_ss - 1 || lane == 31 || snext < 0 || snext == x + 1);   // an unfinished exposure only at the end of a round
               if (sub == n_ss - 1) {
                 W.acc[x & (kAccRing - 1)] = 0;
                 emit1<OutT>(A, row, (uint32_t)e, (double)sum * r.acc_inv, chi);
