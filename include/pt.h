@@ -12,10 +12,14 @@
  *   - Pointers named d_* are DEVICE pointers (e.g. torch tensor .data_ptr()); pointers named h_* are HOST pointers.
  *     The caller owns all of them.  The d_* entry points never allocate, free, copy to the host or synchronise: they
  *     validate their arguments, enqueue kernels on `stream` (a cudaStream_t passed as void*; NULL = default stream)
- *     and return.  They are re-entrant (any thread, any stream).  The only state the library keeps is a ring of 64
- *     scheduler slots in device memory (tile counters of the persistent flux kernel, and room for the per-vector records
- *     of up to 512 parameter vectors); every launch takes the next slot and leaves its counters zeroed, so launches on
- *     different streams do not share one unless more than 64 launches are in flight at once.
+ *     and return.  They are re-entrant (any thread, any stream).  The only state the library keeps is a set of
+ *     scheduler slots in device memory per device (work counters of the persistent kernels, and room for the records,
+ *     row order and transit epochs of up to 4096 parameter vectors).  A launch takes a slot and leaves its counters
+ *     zeroed; 16 slots are shared round-robin, each guarded by an event recorded behind the launch that holds it, and a
+ *     launch that finds all of them in flight makes `stream` wait for the oldest (cudaStreamWaitEvent: ordering on the
+ *     device, no host synchronisation), so two live launches never share one whatever the number of streams.  A launch
+ *     made while `stream` is being captured into a CUDA graph takes one of 8 further slots for good and makes no CUDA
+ *     call other than the kernel launches; when those are used up, capturing returns PT_ERR_CUDA.
  *   - Parameter rows (`d_params`, row-major [n_pv][6 + 3 n_pb] doubles):
  *         [ t0, P, a/R*, i, e, w,  k_0, u1_0, u2_0,  k_1, u1_1, u2_1, ... ]
  *     t0 = time of inferior conjunction, P = period (same unit as the times), a/R* = scaled semi-major axis,
