@@ -130,3 +130,28 @@ def flux_pixels(k: float, z: float, a: float, b: float, n: int = 2000):
     m = 0.5 * (x + 1.0)
     total = 2.0 * np.pi * np.sum(0.5 * w * (1.0 - a * (1.0 - m) - b * (1.0 - m) ** 2) * m)
     return 1.0 - blocked / total
+
+
+def alpha_n_definition(n: int, k: float, z: float):
+    """The Giménez basis function by its definition (Eq. 4 with Eq. 7-8: the flux lost to the μ^n term of the limb
+    darkening law, in units of π): α_n(k, z) = (1/π) ∫_occulted μ^n dA, μ = sqrt(1 - r²), as a 1-D integral over the
+    star-centred radius with the arc of the circle of radius r that lies inside the planet's disk (30-digit tanh-sinh)."""
+    import mpmath as mp
+    mp.mp.dps = 30
+    k, z = mp.mpf(k), mp.mpf(z)
+    lo, hi = max(mp.mpf(0), z - k), min(mp.mpf(1), z + k)
+    if hi <= lo:
+        return mp.mpf(0)
+
+    def arc(r):
+        if r <= k - z:
+            return 2 * mp.pi
+        if r <= z - k or r >= z + k:
+            return mp.mpf(0)
+        return 2 * mp.acos((r * r + z * z - k * k) / (2 * r * z))
+
+    pts = [lo, hi]
+    if k > z and k - z < hi:
+        pts = [lo, k - z, hi]
+    pts = sorted(set(pts + [(pts[0] + pts[-1]) / 2]))
+    return mp.quad(lambda r: (1 - r * r) ** (mp.mpf(n) / 2) * r * arc(r), pts) / mp.pi

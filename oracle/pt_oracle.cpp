@@ -68,6 +68,10 @@ static inline quad x_atanh(quad x) { return atanhq(x); }
 static inline quad x_atan2(quad y, quad x) { return atan2q(y, x); }
 static inline quad x_fabs(quad x) { return fabsq(x); }
 static inline quad x_floor(quad x) { return floorq(x); }
+static inline double x_pow(double x, double y) { return std::pow(x, y); }
+static inline quad x_pow(quad x, quad y) { return powq(x, y); }
+static inline double x_tgamma(double x) { return std::tgamma(x); }
+static inline quad x_tgamma(quad x) { return tgammaq(x); }
 
 template <class R> struct Real;
 template <> struct Real<double> {
@@ -528,6 +532,114 @@ static int table_build_impl(double k_min, double k_max, int n_k, double z_max, i
   return 0;
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// The Giménez model (Eq. 1-12), written out as printed.
+//   f(k,z) = 1 - α(k,z),   α = Σ_{n=0}^{N} C_n α_n(b,c),   b = k/(1+k), c = z/(1+k)                     Eq. 1, 2
+//   α_n(b,c) = b² (1-c²)^{ν+1} / (ν Γ(ν+1)) Σ_{j=0}^{N_J} (-1)^j (2j+ν+2) Γ(ν+j+1)/Γ(j+2)
+//              G_j(ν+2, ν+1; 1-b)² G_j(ν+2, 1; c²),   ν = (n+2)/2                                       Eq. 3
+//   C_0 = (1 - Σ u_n) / (1 - Σ n u_n/(n+2)),  C_n = u_n / (1 - Σ n u_n/(n+2))                           Eq. 7, 8
+//   limb darkening I(μ)/I(1) = 1 - Σ_{n=1}^{N} u_n (1 - μ^n)                                            Eq. 4
+// The paper names G_n(p,q;x) "Jacobi polynomials" without defining them; R20: they are Kopal's (1977), the
+// polynomials of the series the model comes from: G_j(p,q;x) = 2F1(-j, j+p; q; x) = Σ_m (-j)_m (j+p)_m / ((q)_m m!) x^m.
+// With this reading Eq. 3 converges, as N_J grows, to α_n = (1/π) ∫_occulted μ^n dA — the definition that follows from Eq. 4,
+// 7, 8 alone (checked in tests/test_oracle_pins.py against 30-digit quadrature).  Here the polynomial is its defining
+// finite sum, term by term (an alternating sum: use the __float128 instantiation beyond j ~ 25).
+// The defining sum Σ_m (-j)_m (j+p)_m / ((q)_m m!) x^m alternates with terms up to ~1e40 at j = 60 (beyond even __float128), so
+// the same polynomial is evaluated through its other textbook closed form, the two-binomial sum of the Jacobi polynomial it
+// is a multiple of (e.g. Szegő, Orthogonal Polynomials, eq. 4.3.2):
+//   G_j(p,q;x) = j! Γ(q)/Γ(j+q) P_j^{(q-1, p-q)}(1-2x),   P_j^{(α,β)}(1-2x) = Σ_s C(j+α, j-s) C(j+β, s) (-x)^s (1-x)^{j-s},
+// whose terms stay below ~1e16 for x in [0,1] and j <= 60 (C(a,m) = Γ(a+1)/(Γ(m+1)Γ(a-m+1))).  tests/test_oracle_pins.py
+// checks it against mpmath's 2F1 and against the defining sum for small j.
+template <class R> static R gen_binom(R a, int m) { return x_tgamma(a + R(1)) / (x_tgamma(R(m + 1)) * x_tgamma(a - R(m) + R(1))); }
+template <class R> static R kopal_G(int j, R p, R q, R x) {
+  const R al = q - R(1), be = p - q;
+  R sum = R(0);
+  for (int s = 0; s <= j; ++s) {
+    R t = gen_binom<R>(R(j) + al, j - s) * gen_binom<R>(R(j) + be, s) * x_pow(x, R(s)) * x_pow(R(1) - x, R(j - s));
+    sum += (s & 1) ? -t : t;
+  }
+  return x_tgamma(R(j + 1)) * x_tgamma(q) / x_tgamma(R(j) + q) * sum;
+}
+template <class R> static R kopal_G_defining_sum(int j, R p, R q, R x) {
+  R sum = R(1), term = R(1);
+  for (int m = 0; m < j; ++m) {
+    term *= R(m - j) * (R(j) + p + R(m)) / ((q + R(m)) * R(m + 1)) * x;
+    sum += term;
+  }
+  return sum;
+}
+template <class R> static R gimenez_alpha_n(int n, int n_j, R k, R z) {
+  if (!(z < R(1) + k) || !(k > R(0))) return R(0);
+  const R b = k / (R(1) + k), c = z / (R(1) + k);
+  const R nu = R(n + 2) / R(2);
+  R s = R(0);
+  for (int j = 0; j <= n_j; ++j) {
+    const R g1 = kopal_G<R>(j, nu + R(2), nu + R(1), R(1) - b);
+    const R g2 = kopal_G<R>(j, nu + R(2), R(1), c * c);
+    const R a = R((j & 1) ? -1 : 1) * (R(2 * j) + nu + R(2)) * x_tgamma(nu + R(j + 1)) / x_tgamma(R(j + 2));
+    s += a * g1 * g1 * g2;
+  }
+  return b * b * x_pow(R(1) - c * c, nu + R(1)) / (nu * x_tgamma(nu + R(1))) * s;
+}
+// Row layout of the Giménez entry points: [t0, P, a/R*, i, e, w, k,  u_1..u_N (passband 0), u_1..u_N (passband 1), ...].
+static bool gimenez_row_is_valid(const double* pr, int n_pb, int n_ldc) {
+  for (int j = 0; j < 7 + n_pb * n_ldc; ++j) if (!std::isfinite(pr[j])) return false;
+  if (!(pr[1] > 0.0) || !(pr[2] > 0.0) || !(pr[4] >= 0.0 && pr[4] < 1.0) || !(pr[6] >= 0.0)) return false;
+  for (int q = 0; q < n_pb; ++q) {
+    double den = 1.0;
+    for (int n = 1; n <= n_ldc; ++n) den -= n * pr[7 + q * n_ldc + n - 1] / (n + 2.0);
+    if (den == 0.0) return false;
+  }
+  return true;
+}
+template <class R>
+static int gimenez_exact_impl(const double* times, int64_t n_t, int64_t t_stride_pv, const double* params, int64_t n_pv,
+                              int n_pb, int n_ldc, int n_j, int n_ss, double t_exp, double* flux_out) {
+  if (!times || !params || !flux_out) return 1;
+  if (n_t <= 0 || n_pv <= 0 || n_pb < 1 || n_ss < 1 || n_ldc < 1 || n_j < 0) return 2;
+  const int64_t row = 7 + (int64_t)n_pb * n_ldc;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int64_t pv = 0; pv < n_pv; ++pv) {
+    const double* pr = params + pv * row;
+    const double* tt = times + pv * t_stride_pv;
+    double* fo = flux_out + pv * n_pb * n_t;
+    if (!gimenez_row_is_valid(pr, n_pb, n_ldc)) {
+      for (int64_t j = 0; j < n_pb * n_t; ++j) fo[j] = std::numeric_limits<double>::quiet_NaN();
+      continue;
+    }
+    double orow[9] = {pr[0], pr[1], pr[2], pr[3], pr[4], pr[5], pr[6], 0.0, 0.0};
+    Orbit<R> orb(orow);
+    const R k = R(pr[6]);
+    std::vector<R> C((size_t)n_pb * (n_ldc + 1));                      // Eq. 7, 8
+    for (int q = 0; q < n_pb; ++q) {
+      R su = R(0), den = R(1);
+      for (int n = 1; n <= n_ldc; ++n) { const R u = R(pr[7 + q * n_ldc + n - 1]); su += u; den -= R(n) * u / R(n + 2); }
+      C[(size_t)q * (n_ldc + 1)] = (R(1) - su) / den;
+      for (int n = 1; n <= n_ldc; ++n) C[(size_t)q * (n_ldc + 1) + n] = R(pr[7 + q * n_ldc + n - 1]) / den;
+    }
+    std::vector<R> acc(n_pb), an(n_ldc + 1);
+    for (int64_t j = 0; j < n_t; ++j) {
+      for (int q = 0; q < n_pb; ++q) acc[q] = R(0);
+      for (int s = 0; s < n_ss; ++s) {
+        const double ts = subsample_time(tt[j], t_exp, s, n_ss);
+        const R zs = orb.z_signed(fold_phase(ts, pr[0], pr[1]));
+        if (zs >= R(0) && zs < R(1) + k && k > R(0)) {
+          for (int n = 0; n <= n_ldc; ++n) an[n] = gimenez_alpha_n<R>(n, n_j, k, zs);
+          for (int q = 0; q < n_pb; ++q) {
+            R al = R(0);
+            for (int n = 0; n <= n_ldc; ++n) al += C[(size_t)q * (n_ldc + 1) + n] * an[n];   // Eq. 9
+            acc[q] += R(1) - al;
+          } 
+        } else {
+          for (int q = 0; q < n_pb; ++q) acc[q] += R(1);
+        }
+      }
+      for (int q = 0; q < n_pb; ++q) fo[(int64_t)q * n_t + j] = (double)(acc[q] / R(n_ss));
+    }
+  }
+  return 0;
+}
+
 extern "C" {
 
 int pto_num_threads(void) {
@@ -595,6 +707,23 @@ int pto_true_anomaly_series(int prec, int order, const double* M, const double* 
   for (int64_t i = 0; i < n; ++i)
     f[i] = prec == 0 ? true_anomaly_series<double>(M[i], e[i], order) : (double)true_anomaly_series<quad>(quad(M[i]), quad(e[i]), order);
   return 0;
+}
+
+int pto_gimenez_alpha(int prec, int n, int n_j, const double* k, const double* z, int64_t n_pts, double* out) {
+  for (int64_t i = 0; i < n_pts; ++i)
+    out[i] = prec == 0 ? gimenez_alpha_n<double>(n, n_j, k[i], z[i]) : (double)gimenez_alpha_n<quad>(n, n_j, quad(k[i]), quad(z[i]));
+  return 0;
+}
+int pto_kopal_G(int prec, int j, double p, double q, const double* x, int64_t n_pts, double* out) {
+  for (int64_t i = 0; i < n_pts; ++i)
+    out[i] = prec == 0 ? kopal_G<double>(j, p, q, x[i]) : (prec == 1 ? (double)kopal_G<quad>(j, quad(p), quad(q), quad(x[i]))
+                                                                     : (double)kopal_G_defining_sum<quad>(j, quad(p), quad(q), quad(x[i])));
+  return 0;
+}
+int pto_gimenez_exact(int prec, const double* times, int64_t n_t, int64_t t_stride_pv, const double* params, int64_t n_pv,
+                      int32_t n_pb, int32_t n_ldc, int32_t n_j, int32_t n_ss, double t_exp, double* flux_out) {
+  return prec == 0 ? gimenez_exact_impl<double>(times, n_t, t_stride_pv, params, n_pv, n_pb, n_ldc, n_j, n_ss, t_exp, flux_out)
+                   : gimenez_exact_impl<quad>(times, n_t, t_stride_pv, params, n_pv, n_pb, n_ldc, n_j, n_ss, t_exp, flux_out);
 }
 
 int pto_ma_quad_exact(int prec, const double* times, int64_t n_t, int64_t t_stride_pv, const double* params,

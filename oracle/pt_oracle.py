@@ -40,7 +40,7 @@ def lib() -> C.CDLL:
     with _lock:
         if _lib is None:
             _lib = C.CDLL(build())
-            for name in ("pto_ma_basis", "pto_ellip", "pto_kepler", "pto_kepler_iter", "pto_true_anomaly_series", "pto_orbit_z", "pto_orbit_z_solver", "pto_ma_quad_exact",
+            for name in ("pto_ma_basis", "pto_ellip", "pto_kepler", "pto_kepler_iter", "pto_true_anomaly_series", "pto_orbit_z", "pto_orbit_z_solver", "pto_gimenez_alpha", "pto_kopal_G", "pto_gimenez_exact", "pto_ma_quad_exact",
                          "pto_ma_table_build", "pto_ma_quad_interp", "pto_interp_basis", "pto_num_threads"):
                 getattr(_lib, name).restype = C.c_int
             _lib.pto_set_num_threads.restype = None
@@ -239,3 +239,52 @@ def ma_quad_exact_pbk(times, params, n_pb: int = 1, n_ss: int = 1, t_exp: float 
         row = np.concatenate([params[:, :6], params[:, 6 + 3 * j:9 + 3 * j]], axis=1)
         out.append(ma_quad_exact(times, row, 1, n_ss, t_exp, prec)[:, 0])
     return np.stack(out, axis=1)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Giménez model (R20)
+def kopal_G(j: int, p: float, q: float, x, prec: str = "f128"):
+    """Kopal's Jacobi polynomial G_j(p, q; x) = 2F1(-j, j+p; q; x) by its defining finite sum."""
+    x = np.ascontiguousarray(_f64(x))
+    out = np.empty_like(x)
+    lib().pto_kopal_G(C.c_int(2 if prec == "defsum" else PREC[prec]), C.c_int(j), C.c_double(p), C.c_double(q), _p(x), C.c_int64(x.size), _p(out))
+    return out
+
+
+def gimenez_alpha(n: int, n_j: int, k, z, prec: str = "f128"):
+    """α_n(k, z) of Eq. 3 with N_J = n_j terms beyond j = 0."""
+    k, z = np.broadcast_arrays(_f64(k), _f64(z))
+    k, z = np.ascontiguousarray(k), np.ascontiguousarray(z)
+    out = np.empty_like(k)
+    lib().pto_gimenez_alpha(C.c_int(PREC[prec]), C.c_int(n), C.c_int(n_j), _p(k), _p(z), C.c_int64(k.size), _p(out))
+    return out
+
+
+def gimenez_exact(times, params, n_pb: int = 1, n_ldc: int = 2, n_j: int = 40, n_ss: int = 1, t_exp: float = 0.0,
+                  prec: str = "f128"):
+    """Giménez flux [n_pv][n_pb][n_t]; rows [t0, P, a, i, e, w, k, u_1..u_N per passband]."""
+    times, params = np.ascontiguousarray(_f64(times)), np.ascontiguousarray(_f64(params))
+    if params.ndim == 1:
+        params = params[None, :]
+    n_pv = params.shape[0]
+    assert params.shape[1] == 7 + n_pb * n_ldc
+    if times.ndim == 1:
+        n_t, stride = times.shape[0], 0
+    else:
+        assert times.shape[0] == n_pv
+        n_t, stride = times.shape[1], times.shape[1]
+    out = np.empty((n_pv, n_pb, n_t), dtype=np.float64)
+    rc = lib().pto_gimenez_exact(C.c_int(PREC[prec]), _p(times), C.c_int64(n_t), C.c_int64(stride), _p(params), C.c_int64(n_pv),
+                                 C.c_int32(n_pb), C.c_int32(n_ldc), C.c_int32(n_j), C.c_int32(n_ss), C.c_double(t_exp), _p(out))
+    if rc:
+        raise RuntimeError("pto_gimenez_exact failed: %d" % rc)
+    return out
+
+
+def gimenez_interp_alpha(tab_in, tab_out, k: float, z):
+    """The z-interpolation of P:L165-L169 (R21) on given tables of one α_n: tab_in on n_in nodes uniform on
+    [0, 1-k], tab_out on n_out nodes uniform on [1-k, 1+k]; linear interpolation inside the segment that holds z."""
+    z = _f64(z)
+    zi = np.linspace(0.0, 1.0 - k, len(tab_in))
+    zo = np.linspace(1.0 - k, 1.0 + k, len(tab_out))
+    return np.where(z < 1.0 - k, np.interp(z, zi, tab_in), np.interp(z, zo, tab_out))

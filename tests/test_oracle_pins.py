@@ -544,3 +544,59 @@ def test_per_passband_k_mode_pins(oracle):
     q = np.array([[0.0, 3.0, 8.0, np.pi / 2, 0.0, 0.0, 0.1, 0.0, 0.0, 0.2, 0.0, 0.0]])
     f = oracle.ma_quad_exact_pbk(np.array([0.0]), q, 2, prec="f64")
     assert abs(f[0, 0, 0] - (1 - 0.01)) < 1e-15 and abs(f[0, 1, 0] - (1 - 0.04)) < 1e-15
+
+
+# ------------------------------------------------------------------ NEXT-4: the Giménez model
+def test_next4_kopal_polynomials(oracle):
+    # G_j(p,q;x) = 2F1(-j, j+p; q; x) (R20): the oracle's two-binomial evaluation against mpmath's hypergeometric
+    # function and, where that sum is still benign, against the defining sum itself
+    import mpmath as mp
+    mp.mp.dps = 40
+    for j, p, q, x in [(0, 3.0, 2.0, 0.4), (1, 3.5, 2.5, 0.3), (5, 3.5, 2.5, 0.3), (17, 4.0, 1.0, 0.55), (40, 3.5, 2.5, 0.909),
+                       (60, 3.0, 1.0, 0.7), (60, 3.5, 1.0, 0.02), (80, 3.0, 2.0, 0.97)]:
+        ref = mp.hyp2f1(-j, j + p, q, x)
+        got = oracle.kopal_G(j, p, q, [x], "f128")[0]
+        assert abs(got - ref) <= 1e-13 * max(1.0, abs(ref)), (j, p, q, x)
+        if j <= 17:
+            assert abs(oracle.kopal_G(j, p, q, [x], "defsum")[0] - ref) <= 1e-13
+    assert oracle.kopal_G(1, 3.5, 2.5, [0.3], "f128")[0] == pytest.approx(1 - 4.5 * 0.3 / 2.5, abs=1e-15)   # 1 - (1+p) x / q
+
+
+def test_next4_series_converges_to_the_definition(oracle):
+    # Eq. 3 as printed, with Kopal's polynomials, against α_n = (1/π) ∫_occ μ^n dA (the definition that follows from Eq. 4, 7, 8)
+    # by 30-digit quadrature: the error falls as N_J grows (Fig. 1) in every region of (k, z)
+    from oracle.ma_definition import alpha_n_definition
+    for n, k, z in [(0, 0.1, 0.3), (1, 0.1, 0.3), (2, 0.2, 0.9), (1, 0.1, 1.0), (3, 0.15, 0.0), (1, 0.3, 0.75), (4, 0.05, 1.02)]:
+        ref = float(alpha_n_definition(n, k, z))
+        err = [abs(oracle.gimenez_alpha(n, nj, k, z, "f128")[0] - ref) for nj in (5, 40, 100)]
+        # the convergence oscillates (the partial sums overshoot alternately), so the pin is on the envelope
+        assert err[0] > 5 * max(err[1], err[2]), (n, k, z, err)
+        assert err[2] <= 1.5e-6 and err[1] <= 5e-6, (n, k, z, err)
+    # n = 0 and n = 2 have elementary values inside the disk: α_0 = k², α_2 = k² - k²(k² + 2z²)/2
+    a0 = oracle.gimenez_alpha(0, 100, 0.1, 0.4, "f128")[0]
+    a2 = oracle.gimenez_alpha(2, 100, 0.1, 0.4, "f128")[0]
+    assert abs(a0 - 0.01) <= 1e-6 and abs(a2 - (0.01 - 0.01 * (0.01 + 0.32) / 2)) <= 1e-6
+    assert oracle.gimenez_alpha(1, 40, 0.1, 1.1, "f128")[0] == 0.0 and oracle.gimenez_alpha(1, 40, 0.1, 1.3, "f128")[0] == 0.0
+
+
+def test_next4_quadratic_law_reduces_to_mandel_agol(oracle):
+    # N = 2 with u_1 = a + 2b, u_2 = -b is the quadratic law: the Giménez flux tends to the Mandel-Agol flux of the same
+    # oracle (independent code: closed forms + Carlson integrals) as N_J grows; supersampling and two passbands share the α_n
+    t = np.linspace(-0.09, 0.09, 19)
+    a, b = 0.4, 0.2
+    pm = np.array([[0.0, 3.0, 8.0, math.radians(88.0), 0.0, 0.0, 0.1, a, b]])
+    pg = np.array([[0.0, 3.0, 8.0, math.radians(88.0), 0.0, 0.0, 0.1, a + 2 * b, -b, 0.3, 0.0]])   # second passband: linear law u = 0.3
+    fm = oracle.ma_quad_exact(t, pm, prec="f128")[0, 0]
+    pl = pm.copy(); pl[0, 7:] = (0.3, 0.0)
+    fl = oracle.ma_quad_exact(t, pl, prec="f128")[0, 0]
+    errs = []
+    for nj in (5, 40, 80):
+        fg = oracle.gimenez_exact(t, pg, n_pb=2, n_ldc=2, n_j=nj, prec="f128")[0]
+        errs.append(max(np.abs(fg[0] - fm).max(), np.abs(fg[1] - fl).max()))
+    assert errs[0] > 5 * max(errs[1], errs[2]) and errs[1] <= 3e-5 and errs[2] <= 5e-6, errs
+    # out of transit exactly 1; supersampled = mean of the subsample fluxes
+    tt = np.array([0.03, 0.2])
+    f1 = oracle.gimenez_exact(tt, pg, 2, 2, 30, 4, 0.02, prec="f128")
+    offs = 0.02 * ((np.arange(4) + 0.5) / 4 - 0.5)
+    fs = oracle.gimenez_exact((tt[:, None] + offs[None, :]).ravel(), pg, 2, 2, 30, prec="f128").reshape(2, 2, 4).mean(axis=2)
+    assert np.abs(f1[0] - fs).max() <= 1e-15 and np.all(f1[0][:, 1] == 1.0)
