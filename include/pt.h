@@ -163,6 +163,34 @@ int pt_ma_quad_interp_host(const pt_table* table, const double* h_times, int64_t
                            const double* h_params, int64_t n_pv, int32_t n_pb, int32_t n_ss, double t_exp,
                            int32_t dtype, void* h_flux, int32_t* h_status);
 
+/* The Giménez transit model (Eq. 1-12): general limb darkening
+ *   I(μ)/I(1) = 1 - Σ_{n=1}^{N} u_n (1 - μ^n) (Eq. 4),   f = 1 - Σ_{n=0}^{N} C_n α_n(b,c), b = k/(1+k), c = z/(1+k) (Eq. 1, 2),
+ *   α_n = b² (1-c²)^{ν+1} Σ_{j=0}^{n_j} A_{n,j} G_j(ν+2,ν+1;1-b)² G_j(ν+2,1;c²), ν = (n+2)/2 (Eq. 3, 10, 11), C_n from Eq. 7-8,
+ * with the paper's two optimisations: the α_n are evaluated once per sample and combined per passband (Eq. 9), and the
+ * coefficients A_{n,j} and those of the polynomial recurrence are precomputed into a table.  G_j(p,q;x) are
+ * Kopal's Jacobi polynomials 2F1(-j, j+p; q; x) (R20: the paper does not define them).  n_j + 1 terms are summed
+ * (j = 0..n_j); the truncation error falls slowly and oscillates (~1e-5 at n_j = 40, ~1e-6 at 100).
+ *   Parameter rows [n_pv][7 + n_pb*n_ldc]: [t0, P, a/R*, i, e, w, k,  u_1..u_N (passband 0), u_1..u_N (passband 1), ...]
+ *   (one radius ratio; the quadratic law (a, b) is u_1 = a + 2b, u_2 = -b).  Orbit, supersampling, flux layout
+ *   [n_pv][n_pb][n_t] (double), d_status and bad rows (also 1 - Σ n u_n/(n+2) == 0) as for pt_ma_quad_exact.
+ *   Limits: n_ldc <= 8, n_j <= 256, n_pb <= 64 (else PT_ERR_SIZE).
+ * pt_gimenez_coef_size / pt_gimenez_coef_build: the coefficient table, (n_ldc+1)(n_j+1) x 8 doubles in memory the caller
+ *   owns (32-byte aligned), built on the device.
+ * pt_gimenez_exact: every in-transit subsample through the series.
+ * pt_gimenez_interp: the paper's interpolation in z ("first evaluated for n points for z < 1 - k and m points
+ *   for 1 - k < z < k + 1, and the light curve points are interpolated from these tabulated values"; R21): per
+ *   parameter vector, every α_n on n_in nodes uniform on [0, 1-k] and n_out nodes uniform on [1-k, 1+k] (both ends
+ *   included), linear interpolation inside the segment that holds z.  d_work: [n_pv][n_ldc+1][n_in+n_out] doubles owned by
+ *   the caller, filled by the call (one launch) and readable afterwards.  k >= 1 (no inner segment): that row uses the series. */
+int pt_gimenez_coef_size(int32_t n_ldc, int32_t n_j, int64_t* h_bytes);
+int pt_gimenez_coef_build(int32_t n_ldc, int32_t n_j, double* d_coef, void* stream);
+int pt_gimenez_exact(const double* d_coef, int32_t n_ldc, int32_t n_j, const double* d_times, int64_t n_t, int64_t t_stride_pv,
+                     const double* d_params, int64_t n_pv, int32_t n_pb, int32_t n_ss, double t_exp, double* d_flux,
+                     int32_t* d_status, void* stream);
+int pt_gimenez_interp(const double* d_coef, int32_t n_ldc, int32_t n_j, int32_t n_in, int32_t n_out, double* d_work,
+                      const double* d_times, int64_t n_t, int64_t t_stride_pv, const double* d_params, int64_t n_pv,
+                      int32_t n_pb, int32_t n_ss, double t_exp, double* d_flux, int32_t* d_status, void* stream);
+
 /* Diagnostics for the roofline denominator (the FP64 vector-pipe peak is not in MEASURED_PEAKS.json):
  * every thread of `blocks` x 256 runs `iters` rounds of 8 independent DFMA chains and stores one double to
  * d_sink[blocks*256] so the work cannot be removed.  FP64 thread-instructions issued = blocks*256*iters*8. */

@@ -288,3 +288,30 @@ def gimenez_interp_alpha(tab_in, tab_out, k: float, z):
     zi = np.linspace(0.0, 1.0 - k, len(tab_in))
     zo = np.linspace(1.0 - k, 1.0 + k, len(tab_out))
     return np.where(z < 1.0 - k, np.interp(z, zi, tab_in), np.interp(z, zo, tab_out))
+
+
+def gimenez_interp_flux(tables, n_in: int, times, params, n_pb: int = 1, n_ldc: int = 2, n_ss: int = 1, t_exp: float = 0.0):
+    """Flux of the interpolated Giménez model from GIVEN tables [n_pv][n_ldc+1][n_in+n_out] (R21): orbit of this
+    oracle in quad, linear interpolation of every α_n in the segment that holds z, Eq. 7-9, supersample mean."""
+    times, params = _f64(times), _f64(params)
+    n_pv = params.shape[0]
+    tt = np.broadcast_to(times, (n_pv, times.shape[-1])) if times.ndim == 1 else times
+    n_t = tt.shape[1]
+    orow = np.concatenate([params[:, :7], np.zeros((n_pv, 2))], axis=1)
+    z = orbit_z(tt if times.ndim == 2 else times, orow, 1, n_ss, t_exp, prec="f128")          # [n_pv][n_t][n_ss]
+    out = np.ones((n_pv, n_pb, n_t))
+    for pv in range(n_pv):
+        k = params[pv, 6]
+        u = params[pv, 7:].reshape(n_pb, n_ldc)
+        nn = np.arange(1, n_ldc + 1)
+        den = 1.0 - (nn * u / (nn + 2.0)).sum(axis=1)
+        Cc = np.concatenate([((1.0 - u.sum(axis=1)) / den)[:, None], u / den[:, None]], axis=1)      # [n_pb][n_ldc+1]
+        zz = z[pv]
+        intr = (zz >= 0) & (zz < 1.0 + k)
+        an = np.zeros((n_ldc + 1,) + zz.shape)
+        for n in range(n_ldc + 1):
+            an[n] = np.where(intr, gimenez_interp_alpha(tables[pv, n, :n_in], tables[pv, n, n_in:], k, np.abs(zz)), 0.0)
+        abar = an.mean(axis=2)                                                                         # [n_ldc+1][n_t]
+        out[pv] = 1.0 - Cc @ abar
+        out[pv][:, ~intr.any(axis=1)] = 1.0
+    return out

@@ -21,7 +21,8 @@ PT_ST_BAD_PARAM, PT_ST_K_OUT_OF_TABLE = 1, 2
 _ERR = {1: "PT_ERR_NULL", 2: "PT_ERR_SIZE", 3: "PT_ERR_DTYPE", 4: "PT_ERR_TABLE", 5: "PT_ERR_CUDA"}
 
 EXPORTS = ("pt_build_arch", "pt_orbit_z", "pt_orbit_z_solver", "pt_ma_quad_exact", "pt_ma_table_build", "pt_table_spacing", "pt_ma_quad_interp", "pt_ma_quad_chi2", "pt_ma_quad_exact_pbk",
-           "pt_ma_quad_exact_host", "pt_ma_quad_interp_host", "pt_plan", "pt_probe_dfma", "pt_probe_ffma", "pt_launch_count")
+           "pt_ma_quad_exact_host", "pt_ma_quad_interp_host", "pt_plan", "pt_probe_dfma", "pt_probe_ffma",
+           "pt_gimenez_coef_size", "pt_gimenez_coef_build", "pt_gimenez_exact", "pt_gimenez_interp", "pt_launch_count")
 
 
 class PtError(RuntimeError):
@@ -59,6 +60,10 @@ def lib() -> C.CDLL:
         L.pt_ma_quad_exact_host.argtypes = common + [i32, ptr, ptr]
         L.pt_ma_quad_interp_host.argtypes = [C.POINTER(pt_table)] + common + [i32, ptr, ptr]
         L.pt_probe_dfma.argtypes = [i32, i32, ptr, ptr]
+        L.pt_gimenez_coef_size.argtypes = [i32, i32, C.POINTER(i64)]
+        L.pt_gimenez_coef_build.argtypes = [i32, i32, ptr, ptr]
+        L.pt_gimenez_exact.argtypes = [ptr, i32, i32, ptr, i64, i64, ptr, i64, i32, i32, dbl, ptr, ptr, ptr]
+        L.pt_gimenez_interp.argtypes = [ptr, i32, i32, i32, i32, ptr, ptr, i64, i64, ptr, i64, i32, i32, dbl, ptr, ptr, ptr]
         L.pt_probe_ffma.argtypes = [i32, i32, ptr, ptr]
         L.pt_plan.argtypes = [i64, i64, i32, C.POINTER(C.c_int64)]
         for n in EXPORTS[1:-1]:
@@ -235,6 +240,64 @@ def pt_ma_quad_interp_host(table: Table, times: torch.Tensor, params: torch.Tens
                                         n_pb, n_ss, float(t_exp), _dtype_code(out.dtype), out.data_ptr(),
                                         status.data_ptr() if status is not None else None), "pt_ma_quad_interp_host")
     return out
+
+
+class GimenezCoef:
+    """The coefficient table of the Giménez model for (n_ldc, n_j), built on the device (include/pt.h: pt_gimenez_coef_build)."""
+
+    def __init__(self, n_ldc: int, n_j: int, device=None):
+        nbytes = C.c_int64(0)
+        _check(lib().pt_gimenez_coef_size(n_ldc, n_j, C.byref(nbytes)), "pt_gimenez_coef_size")
+        self.n_ldc, self.n_j = int(n_ldc), int(n_j)
+        self.data = torch.empty(nbytes.value // 8, dtype=torch.float64, device=device or torch.device("cuda", torch.cuda.current_device()))
+        _check(lib().pt_gimenez_coef_build(n_ldc, n_j, self.data.data_ptr(), _stream()), "pt_gimenez_coef_build")
+
+
+def _marshal_gimenez(times, params, n_pb, n_ldc):
+    if params.dim() == 1:
+        params = params[None, :]
+    if times.dtype != torch.float64 or params.dtype != torch.float64 or not (times.is_contiguous() and params.is_contiguous()):
+        raise PtError("times and params must be contiguous float64")
+    if not (times.is_cuda and params.is_cuda):
+        raise PtError("times and params must be CUDA tensors (there is no CPU path)")
+    n_pv = params.shape[0]
+    if params.shape[1] != 7 + n_pb * n_ldc:
+        raise PtError("Giménez parameter rows must hold 7 + n_pb*n_ldc doubles")
+    if times.dim() == 1:
+        n_t, stride = times.shape[0], 0
+    elif times.dim() == 2 and times.shape[0] == n_pv:
+        n_t, stride = times.shape[1], times.shape[1]
+    else:
+        raise PtError("times must be [n_t] or [n_pv][n_t]")
+    return times, params, n_pv, n_t, stride
+
+
+def pt_gimenez_exact(coef: GimenezCoef, times: torch.Tensor, params: torch.Tensor, n_pb: int = 1, n_ss: int = 1,
+                     t_exp: float = 0.0, out: Optional[torch.Tensor] = None, status: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """Giménez flux [n_pv][n_pb][n_t] by the series (include/pt.h: pt_gimenez_exact)."""
+    times, params, n_pv, n_t, stride = _marshal_gimenez(times, params, n_pb, coef.n_ldc)
+    if out is None:
+        out = torch.empty((n_pv, n_pb, n_t), dtype=torch.float64, device=times.device)
+    _check(lib().pt_gimenez_exact(coef.data.data_ptr(), coef.n_ldc, coef.n_j, times.data_ptr(), n_t, stride, params.data_ptr(),
+                                  n_pv, n_pb, n_ss, float(t_exp), out.data_ptr(),
+                                  status.data_ptr() if status is not None else None, _stream()), "pt_gimenez_exact")
+    return out
+
+
+def pt_gimenez_interp(coef: GimenezCoef, n_in: int, n_out: int, times: torch.Tensor, params: torch.Tensor, n_pb: int = 1,
+                      n_ss: int = 1, t_exp: float = 0.0, out: Optional[torch.Tensor] = None,
+                      work: Optional[torch.Tensor] = None, status: Optional[torch.Tensor] = None):
+    """Giménez flux by interpolation in z (include/pt.h: pt_gimenez_interp); returns (flux, work) — work holds the tables
+    [n_pv][n_ldc+1][n_in+n_out] the call filled."""
+    times, params, n_pv, n_t, stride = _marshal_gimenez(times, params, n_pb, coef.n_ldc)
+    if out is None:
+        out = torch.empty((n_pv, n_pb, n_t), dtype=torch.float64, device=times.device)
+    if work is None:
+        work = torch.empty((n_pv, coef.n_ldc + 1, n_in + n_out), dtype=torch.float64, device=times.device)
+    _check(lib().pt_gimenez_interp(coef.data.data_ptr(), coef.n_ldc, coef.n_j, n_in, n_out, work.data_ptr(), times.data_ptr(),
+                                   n_t, stride, params.data_ptr(), n_pv, n_pb, n_ss, float(t_exp), out.data_ptr(),
+                                   status.data_ptr() if status is not None else None, _stream()), "pt_gimenez_interp")
+    return out, work
 
 
 def pt_probe_ffma(blocks: int, iters: int, sink: torch.Tensor) -> None:

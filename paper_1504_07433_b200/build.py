@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpt_b200.so")
 SOURCES = [os.path.join(CSRC, "pt_kernels.cu")]
-HEADERS = [os.path.join(CSRC, "pt_epoch.cuh"), os.path.join(CSRC, "pt_direct.cuh"), os.path.join(CSRC, "pt_basis32.cuh"), os.path.join(CSRC, "pt_basis.cuh"), os.path.join(CSRC, "pt_orbit.cuh"), os.path.join(CSRC, "pt_math.cuh"), os.path.join(CSRC, "pt_flux.cuh"),
+HEADERS = [os.path.join(CSRC, "pt_gimenez.cuh"), os.path.join(CSRC, "pt_epoch.cuh"), os.path.join(CSRC, "pt_direct.cuh"), os.path.join(CSRC, "pt_basis32.cuh"), os.path.join(CSRC, "pt_basis.cuh"), os.path.join(CSRC, "pt_orbit.cuh"), os.path.join(CSRC, "pt_math.cuh"), os.path.join(CSRC, "pt_flux.cuh"),
            os.path.join(HERE, "..", "include", "pt.h")]
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-DPT_BUILD_ARCH=100",

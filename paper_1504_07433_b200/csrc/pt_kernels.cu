@@ -12,6 +12,7 @@
 #include "pt_flux.cuh"
 #include "pt_epoch.cuh"
 #include "pt_direct.cuh"
+#include "pt_gimenez.cuh"
 
 namespace pt {
 
@@ -588,6 +589,68 @@ int pt_ma_quad_chi2(const pt_table* table, const double* d_times, int64_t n_t, c
   const Chi2Args like{d_obs, d_isig};
   return launch_flux(table ? 1 : 0, table, d_times, n_t, 0, d_params, n_pv, n_pb, n_ss, t_exp, kDtypeChi2, d_chi2, d_status,
                      (cudaStream_t)stream, &like);
+}
+
+// ---- the Giménez model
+int pt_gimenez_coef_size(int32_t n_ldc, int32_t n_j, int64_t* h_bytes) {
+  if (!h_bytes) return PT_ERR_NULL;
+  if (n_ldc < 1 || n_ldc > kGimMaxLdc || n_j < 0 || n_j > kGimMaxNj) return PT_ERR_SIZE;
+  *h_bytes = (int64_t)(n_ldc + 1) * (n_j + 1) * kGimCoef * (int64_t)sizeof(double);
+  return PT_OK;
+}
+
+int pt_gimenez_coef_build(int32_t n_ldc, int32_t n_j, double* d_coef, void* stream) {
+  if (!d_coef) return PT_ERR_NULL;
+  if (n_ldc < 1 || n_ldc > kGimMaxLdc || n_j < 0 || n_j > kGimMaxNj) return PT_ERR_SIZE;
+  if (reinterpret_cast<uintptr_t>(d_coef) % 32 != 0) return PT_ERR_SIZE;
+  const int n = (n_ldc + 1) * (n_j + 1);
+  gimenez_coef_kernel<<<(n + 127) / 128, 128, 0, (cudaStream_t)stream>>>(n_ldc, n_j, d_coef);
+  g_launches.fetch_add(1);
+  return cudaGetLastError() == cudaSuccess ? PT_OK : PT_ERR_CUDA;
+}
+
+static int gimenez_launch(int mode, const double* d_coef, int32_t n_ldc, int32_t n_j, int32_t n_in, int32_t n_out, double* d_work,
+                          const double* d_times, int64_t n_t, int64_t t_stride_pv, const double* d_params, int64_t n_pv,
+                          int32_t n_pb, int32_t n_ss, double t_exp, double* d_flux, int32_t* d_status, void* stream) {
+  if (!d_coef || !d_times || !d_params || !d_flux || (mode == 1 && !d_work)) return PT_ERR_NULL;
+  if (n_t <= 0 || n_pv <= 0 || n_pb < 1 || n_pb > kGimMaxPb || n_ss < 1 || n_ldc < 1 || n_ldc > kGimMaxLdc || n_j < 0 ||
+      n_j > kGimMaxNj || (t_stride_pv != 0 && t_stride_pv < n_t) || (mode == 1 && (n_in < 2 || n_out < 2)))
+    return PT_ERR_SIZE;
+  if (reinterpret_cast<uintptr_t>(d_coef) % 32 != 0) return PT_ERR_SIZE;
+  GimArgs A{};
+  A.coef = d_coef; A.n_ldc = n_ldc; A.n_j = n_j; A.times = d_times; A.n_t = n_t; A.t_stride_pv = t_stride_pv;
+  A.params = d_params; A.n_pv = n_pv; A.n_pb = n_pb; A.n_ss = n_ss; A.t_exp = t_exp; A.flux = d_flux; A.status = d_status;
+  A.work = d_work; A.n_in = n_in; A.n_out = n_out;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (mode == 1) {
+    const int64_t nn = n_pv * (int64_t)(n_in + n_out);
+    if ((nn + 255) / 256 > 0x7fffffff) return PT_ERR_SIZE;
+    gimenez_table_kernel<<<(unsigned)((nn + 255) / 256), 256, 0, st>>>(A);
+    g_launches.fetch_add(1);
+  }
+  int64_t bpp = (n_t + 255) / 256;
+  const int64_t cap = ((int64_t)sm_count() * 16 + n_pv - 1) / n_pv;
+  if (bpp > cap) bpp = cap;
+  if (bpp < 1) bpp = 1;
+  if (n_pv * bpp > 0x7fffffff) return PT_ERR_SIZE;
+  if (mode == 0) gimenez_kernel<0><<<(unsigned)(n_pv * bpp), 256, 0, st>>>(A, (int)bpp);
+  else gimenez_kernel<1><<<(unsigned)(n_pv * bpp), 256, 0, st>>>(A, (int)bpp);
+  g_launches.fetch_add(1);
+  return cudaGetLastError() == cudaSuccess ? PT_OK : PT_ERR_CUDA;
+}
+
+int pt_gimenez_exact(const double* d_coef, int32_t n_ldc, int32_t n_j, const double* d_times, int64_t n_t, int64_t t_stride_pv,
+                     const double* d_params, int64_t n_pv, int32_t n_pb, int32_t n_ss, double t_exp, double* d_flux,
+                     int32_t* d_status, void* stream) {
+  return gimenez_launch(0, d_coef, n_ldc, n_j, 0, 0, nullptr, d_times, n_t, t_stride_pv, d_params, n_pv, n_pb, n_ss, t_exp,
+                        d_flux, d_status, stream);
+}
+
+int pt_gimenez_interp(const double* d_coef, int32_t n_ldc, int32_t n_j, int32_t n_in, int32_t n_out, double* d_work,
+                      const double* d_times, int64_t n_t, int64_t t_stride_pv, const double* d_params, int64_t n_pv,
+                      int32_t n_pb, int32_t n_ss, double t_exp, double* d_flux, int32_t* d_status, void* stream) {
+  return gimenez_launch(1, d_coef, n_ldc, n_j, n_in, n_out, d_work, d_times, n_t, t_stride_pv, d_params, n_pv, n_pb, n_ss,
+                        t_exp, d_flux, d_status, stream);
 }
 
 // ---- host-buffer forms: H2D, kernels, D2H on an internal stream, then wait.

@@ -771,3 +771,93 @@ def test_max_passbands_and_many_subsamples(pt, oracle):
     w = inputs.config2(n_pv=2, n_t=300)
     w.n_ss, w.t_exp = 1500, 0.05
     assert np.abs(gpu_exact(pt, w) - ora_exact(oracle, w)).max() <= TOL64
+
+
+# ------------------------------------------------------------------------------------------- NEXT-4: the Giménez model
+def _gimenez_population(n_pv, n_pb, n_ldc, seed):
+    rng = np.random.default_rng(seed)
+    P, a = rng.uniform(1, 10, n_pv), rng.uniform(4, 20, n_pv)
+    e = np.where(rng.uniform(size=n_pv) < 0.5, 0.0, rng.uniform(0, 0.5, n_pv))
+    wv = rng.uniform(0, 2 * math.pi, n_pv)
+    inc = np.arccos(np.clip(rng.uniform(0, 0.9, n_pv) * (1 + e * np.sin(wv)) / (a * (1 - e * e)), -1, 1))
+    k = rng.uniform(0.02, 0.3, n_pv)
+    u = rng.uniform(-0.1, 0.5, (n_pv, n_pb * n_ldc)) / n_ldc
+    return np.concatenate([np.stack([P * rng.uniform(0, 1, n_pv), P, a, inc, e, wv, k], 1), u], 1)
+
+
+@pytest.mark.parametrize("n_pb,n_ldc,n_j,n_ss", [(1, 2, 40, 1), (3, 2, 25, 1), (2, 4, 30, 3), (1, 1, 60, 1), (2, 8, 10, 1)])
+def test_gimenez_exact_parity(pt, oracle, n_pb, n_ldc, n_j, n_ss):
+    """The series of Eq. 3 with the same N_J on both sides: the kernel runs the polynomials up by the three-term recurrence in
+    fp64 from a precomputed table, the oracle sums each polynomial explicitly in __float128.  Tolerance 1e-11 absolute: the
+    recurrences are stable inside [-1, 1] (error growth ~ j ulp), N_J <= 60 terms of size <= 1e-2 each."""
+    n_pv, n_t = 12, 120
+    params = _gimenez_population(n_pv, n_pb, n_ldc, 50 + n_ldc)
+    rng = np.random.default_rng(7)
+    t14 = params[:, 1] / (math.pi * params[:, 2])
+    t = params[:, 0][:, None] + params[:, 1][:, None] * rng.integers(0, 5, (n_pv, 1)) + rng.uniform(-1.5, 1.5, (n_pv, n_t)) * t14[:, None]
+    params[5, 1] = -1.0
+    coef = pt.GimenezCoef(n_ldc, n_j)
+    st = torch.zeros(2, dtype=torch.int32, device="cuda")
+    f = pt.pt_gimenez_exact(coef, dev(t), dev(params), n_pb, n_ss, 0.01, status=st).cpu().numpy()
+    r = oracle.gimenez_exact(t, params, n_pb, n_ldc, n_j, n_ss, 0.01, prec="f128")
+    assert np.array_equal(np.isnan(f), np.isnan(r)) and np.all(np.isnan(f[5])) and st.cpu().tolist() == [pt.PT_ST_BAD_PARAM, 1]
+    ok = ~np.isnan(r)
+    assert np.abs(f[ok] - r[ok]).max() <= 1e-11
+    assert np.array_equal(f[ok] == 1.0, r[ok] == 1.0) and (r[ok] < 1.0).mean() > 0.3
+
+
+def test_gimenez_quadratic_law_against_mandel_agol(pt, oracle):
+    # N = 2, u_1 = a + 2b, u_2 = -b: the Giménez kernel against the Mandel-Agol kernel and oracle (truncation error, falling with N_J)
+    w = inputs.config2(n_pv=6, n_t=4000)
+    pm = w.params
+    pg = np.concatenate([pm[:, :7], (pm[:, 7] + 2 * pm[:, 8])[:, None], -pm[:, 8][:, None]], axis=1)
+    fm = gpu_exact(pt, inputs.Workload("m", w.times, pm))[:, 0]
+    errs = []
+    for n_j in (10, 40, 160):
+        fg = pt.pt_gimenez_exact(pt.GimenezCoef(2, n_j), dev(w.times), dev(pg)).cpu().numpy()[:, 0]
+        errs.append(np.abs(fg - fm).max())
+        assert np.array_equal(fg == 1.0, fm == 1.0)
+    assert errs[0] > 3 * errs[1] > 9 * errs[2] and errs[1] <= 5e-5 and errs[2] <= 6e-6, errs
+
+
+def test_gimenez_interp_parity(pt, oracle):
+    """the tables the call leaves in d_work against the oracle's α_n at the nodes, and the flux against the
+    oracle's interpolation of THE SAME tables (1e-12); the error against the series is reported, not gated."""
+    n_pv, n_pb, n_ldc, n_j, n_in, n_out, n_t = 6, 2, 2, 30, 40, 60, 400
+    params = _gimenez_population(n_pv, n_pb, n_ldc, 91)
+    rng = np.random.default_rng(8)
+    t14 = params[:, 1] / (math.pi * params[:, 2])
+    t = params[:, 0][:, None] + rng.uniform(-1.2, 1.2, (n_pv, n_t)) * t14[:, None]
+    coef = pt.GimenezCoef(n_ldc, n_j)
+    for n_ss in (1, 3):
+        f, work = pt.pt_gimenez_interp(coef, n_in, n_out, dev(t), dev(params), n_pb, n_ss, 0.004)
+        f, tab = f.cpu().numpy(), work.cpu().numpy()
+        r = oracle.gimenez_interp_flux(tab, n_in, t, params, n_pb, n_ldc, n_ss, 0.004)
+        assert np.abs(f - r).max() <= 1e-12
+    for pv in (0, 3):
+        k = params[pv, 6]
+        zn = np.concatenate([np.linspace(0, 1 - k, n_in), np.linspace(1 - k, 1 + k, n_out)])
+        for n in range(n_ldc + 1):
+            ref = oracle.gimenez_alpha(n, n_j, k, zn, "f128")
+            ref[-1] = 0.0
+            assert np.abs(tab[pv, n] - ref).max() <= 1e-12
+    fx = pt.pt_gimenez_exact(coef, dev(t), dev(params), n_pb, 3, 0.004).cpu().numpy()
+    print("gimenez interp vs series: max %.2e mean %.2e" % (np.abs(f - fx).max(), np.abs(f - fx).mean()))
+    assert np.abs(f - fx).max() <= 1e-3
+
+
+def test_gimenez_argument_errors(pt):
+    from paper_1504_07433_b200 import binding
+    L = binding.lib()
+    import ctypes as C
+    nb = C.c_int64(0)
+    assert L.pt_gimenez_coef_size(2, 40, C.byref(nb)) == 0 and nb.value == 3 * 41 * 8 * 8
+    assert L.pt_gimenez_coef_size(9, 40, C.byref(nb)) == binding.PT_ERR_SIZE
+    assert L.pt_gimenez_coef_size(2, 257, C.byref(nb)) == binding.PT_ERR_SIZE
+    coef = pt.GimenezCoef(2, 10)
+    t = torch.zeros(8, dtype=torch.float64, device="cuda")
+    p = torch.zeros((1, 9), dtype=torch.float64, device="cuda")
+    o = torch.zeros(8, dtype=torch.float64, device="cuda")
+    assert L.pt_gimenez_exact(None, 2, 10, t.data_ptr(), 8, 0, p.data_ptr(), 1, 1, 1, 0.0, o.data_ptr(), None, None) == binding.PT_ERR_NULL
+    assert L.pt_gimenez_exact(coef.data.data_ptr(), 2, 10, t.data_ptr(), 8, 0, p.data_ptr(), 1, 65, 1, 0.0, o.data_ptr(), None, None) == binding.PT_ERR_SIZE
+    assert L.pt_gimenez_interp(coef.data.data_ptr(), 2, 10, 1, 5, o.data_ptr(), t.data_ptr(), 8, 0, p.data_ptr(), 1, 1, 1, 0.0, o.data_ptr(), None, None) == binding.PT_ERR_SIZE
