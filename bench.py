@@ -397,6 +397,27 @@ def run_ours(args):
         res_o["config5"]["orbit_solvers"] = sol
         extra["configs"] = res_o
         del a1, b1, o1, a3, b3, o3, a5, b5, o5, zo
+    if rank == 0 and "gimenez" in sections:
+        # -------------------------------------------------------------- the Giménez model (S§8(f) NEXT-4): series and z-interpolation
+        wg = inputs.dense_transit(n_pv=1024, n_t=4096)
+        pg = np.concatenate([wg.params[:, :7], (wg.params[:, 7] + 2 * wg.params[:, 8])[:, None], -wg.params[:, 8][:, None]], axis=1)
+        gt, gp = to_dev(wg.times), to_dev(pg)
+        go = torch.empty((wg.n_pv, 1, wg.n_t), dtype=torch.float64, device=dev)
+        res_g = {"workload": "1024 pv x 4096 per-pv times near transit (the `dense` population), quadratic law as N = 2, one passband"}
+        for n_j in (20, 40):
+            coef = pt.GimenezCoef(2, n_j)
+            tg = _time_steps(lambda: pt.pt_gimenez_exact(coef, gt, gp, out=go), 5, 2, flush, 1) / 5
+            res_g["series_nj%d" % n_j] = {"value": wg.n_eval / tg, "unit": UNIT, "ms": tg * 1e3}
+        gw = torch.empty((wg.n_pv, 3, 256 + 256), dtype=torch.float64, device=dev)
+        tgi = _time_steps(lambda: pt.pt_gimenez_interp(coef, 256, 256, gt, gp, out=go, work=gw), 5, 2, flush, 1) / 5
+        res_g["interp_256_256_nj40"] = {"value": wg.n_eval / tgi, "unit": UNIT, "ms": tgi * 1e3}
+        fm = pt.pt_ma_quad_exact(gt[:64].contiguous(), to_dev(wg.params[:64]))
+        fgx = pt.pt_gimenez_exact(coef, gt[:64].contiguous(), gp[:64].contiguous())
+        fgi, _ = pt.pt_gimenez_interp(coef, 256, 256, gt[:64].contiguous(), gp[:64].contiguous())
+        res_g["max_abs_diff_series_nj40_vs_mandel_agol"] = float((fgx - fm).abs().max().item())
+        res_g["max_abs_diff_interp_vs_series"] = float((fgi - fgx).abs().max().item())
+        extra["gimenez"] = res_g
+        del gt, gp, go, gw
     if rank == 0 and "chi2" in sections:
         # -------------------------------------------------------------- fused likelihood (S§8(f) NEXT-1): no flux is written
         res_c = {}
@@ -591,8 +612,8 @@ def main():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--sections", default="scaled,dense,interp,configs,chi2,cpu",
-                    help="extra sections to run besides the headline: any of scaled,dense,interp,configs,chi2,cpu (or 'none')")
+    ap.add_argument("--sections", default="scaled,dense,interp,configs,chi2,gimenez,cpu",
+                    help="extra sections to run besides the headline: any of scaled,dense,interp,configs,chi2,gimenez,cpu (or 'none')")
     ap.add_argument("--workload", default=None, help="run only this workload (%s): the command of the ncu captures" % ", ".join(WORKLOADS))
     args = ap.parse_args()
     if args.workload:
