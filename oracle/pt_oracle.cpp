@@ -15,6 +15,8 @@
 //   supersampling: mean of n evenly distributed subsamples inside each exposure
 //   interpolated model: bilinear interpolation in (k,z) tables of λe, λd, ηd
 //   orbit: circular, and eccentric by a Kepler solve (paper names the solvers only)
+//   the other orbit routines: fixed-point iteration, two series, e-based dispatch      P:L31 (R19)
+//   the Giménez model with general limb darkening, Eq. 1-12 as printed                 P:L40-L128 (R20)
 //
 // Method choices that are deliberately DIFFERENT from the CUDA path (so that a shared mistake is unlikely):
 //   * elliptic integrals K, E, Π by Carlson's symmetric forms R_F, R_D, R_J (duplication), not Bulirsch cel;
