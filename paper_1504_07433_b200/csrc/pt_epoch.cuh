@@ -36,6 +36,9 @@
 
 namespace pt {
 
+#ifndef PT_EPOCH_WARPS
+#define PT_EPOCH_WARPS 24   // single-warp blocks per SM of the exact model's epoch kernel
+#endif
 constexpr int kAccRing = 64;        // supersample accumulators in flight per warp (exposures are finished in order)
 constexpr int kBcumMax = 4096;      // rows of a launch the epoch kernel takes (= the slot's record capacity)
 constexpr int kOffTable = 256;      // subsample offsets tabulated per block (n_ss up to this; computed on the fly above)
@@ -163,7 +166,7 @@ __device__ __forceinline__ void stage_table(const FluxArgs& A, const PvRec& r, d
 // MODE 0: exact (NT = 32: a block is one autonomous warp).  MODE 1: interpolated (NT = 512; exact basis functions for a
 // parameter vector whose k̂ is off the table).  V2: rows allow aligned pair stores.  SS1: n_ss == 1.
 template <int MODE, int NT, bool V2, bool SS1, typename OutT>
-__global__ void __launch_bounds__(NT, (NT == 32 ? 24 : 2)) epoch_kernel(const __grid_constant__ FluxArgs A) {
+__global__ void __launch_bounds__(NT, (NT == 32 ? PT_EPOCH_WARPS : 2)) epoch_kernel(const __grid_constant__ FluxArgs A) {
   extern __shared__ double s_G[];                       // MODE 1: the staged table of the current unit, n_z doubles
   __shared__ EpochWarp s_w[SS1 ? 1 : NT / 32];
   __shared__ double s_off[SS1 ? 1 : kOffTable];

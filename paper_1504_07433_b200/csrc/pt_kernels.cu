@@ -376,12 +376,15 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   // epoch kernel: interpolated model = blocks of 16 warps that stage the table (n_z doubles of shared memory, two per SM);
   // exact model = single-warp blocks, 24 per SM.  About four units per block so that the ticket counter balances the load.
   const int e_nt = (mode == 1) ? 512 : 32;
-  const int64_t e_grid = (int64_t)sm_count() * ((mode == 1) ? 2 : 24);
+  const int64_t e_grid = (int64_t)sm_count() * ((mode == 1) ? 2 : PT_EPOCH_WARPS);
   const size_t e_smem = (mode == 1) ? (size_t)tb->n_z * sizeof(double) : 0;
   if (want_epoch) {
     Q.want_units = 1; Q.un0 = slot->un0; Q.ucnt = slot->ucnt; Q.n_blocks = n_prep;
     A.un0 = slot->un0; A.ucnt = slot->ucnt;
-    int64_t C = (4 * e_grid + n_pv - 1) / n_pv;
+#ifndef PT_EPOCH_UNITS
+#define PT_EPOCH_UNITS 4
+#endif
+    int64_t C = (PT_EPOCH_UNITS * e_grid + n_pv - 1) / n_pv;
     A.unit_chunks = (int)(C < 1 ? 1 : (C > 4096 ? 4096 : C));
     A.base_added = (dtype == kDtypeChi2) ? 1 : 0;
   }
