@@ -12,6 +12,8 @@
 // front of each of them: epoch j owns the exposures [hi_{j-1}, hi_j) — the gap before its window, written as pure 16-byte
 // streaming stores (no time loads, no arithmetic), and its window, every exposure of which is evaluated.  hi_{-1} = 0 and
 // the last epoch of the row also owns the tail, so the units partition the output exactly and nothing is searched twice.
+// (A batch of epochs writes its ones as ONE run over its whole stretch and then overwrites the windows — same warp, ordered by
+// a __syncwarp — instead of one short run per gap: 4 % more bytes, a tenth of the fill instructions; PT_FILL_THROUGH.)
 // Units are dealt to the blocks of one persistent grid from a ticket counter, rows in the order prep_kernel left (by k̂
 // for the table: neighbouring tickets read neighbouring table rows; heaviest first for the exact model).
 //
@@ -36,6 +38,10 @@
 
 namespace pt {
 
+#ifndef PT_FILL_THROUGH
+#define PT_FILL_THROUGH 1     // 1: a batch writes ones over its whole stretch and overwrites the windows (0.737 -> 0.704 ms on configs[3]);
+                               // 0: only the gaps are filled, every element is written exactly once
+#endif
 #ifndef PT_EPOCH_WARPS
 #define PT_EPOCH_WARPS 24   // single-warp blocks per SM of the exact model's epoch kernel
 #endif
@@ -272,6 +278,16 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? PT_EPOCH_WARPS : 2)) epoch_ker
         int phi = __shfl_up_sync(0xffffffffu, hi, 1);
         const int phi0 = __shfl_sync(0xffffffffu, hi, m);
         if (lane == 0) phi = phi0;
+#if PT_FILL_THROUGH
+        // one long run of ones over the whole stretch of the batch, windows included; the evaluation below overwrites the
+        // windows (same warp, ordered by the __syncwarp): a few per cent more bytes, a tenth of the fill instructions
+        if constexpr (!kIsChi2<OutT>) {
+          const int hl = __shfl_sync(0xffffffffu, hi, m - 1);
+          fill_span<V2, OutT>(row, (uint32_t)phi0, (uint32_t)((first + (uint32_t)m == cnt) ? n_t : hl), (OutT)1.0);
+          __syncwarp();
+        }
+        (void)phi;
+#else
         for (int i = 0; i < m; ++i) {
           const int a = __shfl_sync(0xffffffffu, phi, i), b = __shfl_sync(0xffffffffu, lo, i);
           PT_CHECK(a >= 0 && b <= n_t);                      // a > b never happens (the windows are disjoint) and would be a no-op
@@ -280,6 +296,7 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? PT_EPOCH_WARPS : 2)) epoch_ker
         if constexpr (!kIsChi2<OutT>) {
           if (first + (uint32_t)m == cnt) fill_span<V2, OutT>(row, (uint32_t)__shfl_sync(0xffffffffu, hi, m - 1), (uint32_t)n_t, (OutT)1.0);   // tail of the row
         }
+#endif
         // in-window exposures of the batch, packed over the lanes
         const int rcnt = lane < m ? hi - lo : 0;
         int cum = rcnt;                                   // inclusive scan of the range lengths

@@ -60,7 +60,7 @@ __device__ __forceinline__ void gimenez_alphas(const double* __restrict__ coef, 
     double p1m = 0.0, p1 = 1.0, p2m = 0.0, p2 = 1.0, s = 0.0;
     for (int j = 0; j <= n_j; ++j) {
       const double2* cj = (const double2*)(cf + (size_t)j * kGimCoef);     // the same address in every lane: a broadcast
-      const double2 qa = __ldg(cj), qb = __ldg(cj + 1), qc = __ldg(cj + 2), qd = __ldg(cj + 3);
+      const double2 qa = cj[0], qb = cj[1], qc = cj[2], qd = cj[3];          // read-only: global (L1) or shared memory
       s = fma(qa.x * p1 * p1, p2, s);                                         // B P1² P2
       const double n1 = fma(fma(qb.x, y1, qa.y), p1, -qb.y * p1m);            // r1 = (qa.y, qb.x, qb.y)
       const double n2 = fma(fma(qc.y, y2, qc.x), p2, -qd.x * p2m);            // r2 = (qc.x, qc.y, qd.x)
@@ -106,9 +106,16 @@ __device__ __forceinline__ void gimenez_setup(const GimArgs& A, const double* ro
 
 // MODE 0: every in-transit subsample through the series.  MODE 1: linear interpolation in the per-vector z-tables of `work`.
 template <int MODE>
-__global__ void __launch_bounds__(256) gimenez_kernel(const __grid_constant__ GimArgs A, int blocks_per_pv) {
+__global__ void __launch_bounds__(256) gimenez_kernel(const __grid_constant__ GimArgs A, int blocks_per_pv, int coef_in_smem) {
+  extern __shared__ double2 s_coef2[];                  // the coefficient table, when it fits (MODE 0)
   __shared__ PvConst c;
   __shared__ double C[kGimMaxPb * (kGimMaxLdc + 1)];
+  const double* coef = A.coef;
+  if (MODE == 0 && coef_in_smem) {
+    const int n2 = (A.n_ldc + 1) * (A.n_j + 1) * kGimCoef / 2;
+    for (int i = threadIdx.x; i < n2; i += blockDim.x) s_coef2[i] = __ldg((const double2*)A.coef + i);
+    coef = reinterpret_cast<const double*>(s_coef2);
+  }
   const int64_t pv = blockIdx.x / blocks_per_pv;
   const int chunk = (int)(blockIdx.x % blocks_per_pv);
   const int64_t rowlen = 7 + (int64_t)A.n_pb * A.n_ldc;
@@ -155,7 +162,7 @@ __global__ void __launch_bounds__(256) gimenez_kernel(const __grid_constant__ Gi
               an[n] = fma(f, v1 - v0, v0);
             }
           } else {
-            gimenez_alphas(A.coef, A.n_ldc, A.n_j, k, zs, an);
+            gimenez_alphas(coef, A.n_ldc, A.n_j, k, zs, an);
           }
           for (int n = 0; n <= A.n_ldc; ++n) acc[n] += an[n];
         }

@@ -636,8 +636,11 @@ static int gimenez_launch(int mode, const double* d_coef, int32_t n_ldc, int32_t
   if (bpp > cap) bpp = cap;
   if (bpp < 1) bpp = 1;
   if (n_pv * bpp > 0x7fffffff) return PT_ERR_SIZE;
-  if (mode == 0) gimenez_kernel<0><<<(unsigned)(n_pv * bpp), 256, 0, st>>>(A, (int)bpp);
-  else gimenez_kernel<1><<<(unsigned)(n_pv * bpp), 256, 0, st>>>(A, (int)bpp);
+  // the series reads the coefficient table (n_ldc+1)(n_j+1) x 64 bytes once per term: from shared memory when it fits
+  const size_t coef_bytes = (size_t)(n_ldc + 1) * (n_j + 1) * kGimCoef * sizeof(double);
+  const int in_smem = (mode == 0 && coef_bytes <= 40 * 1024) ? 1 : 0;
+  if (mode == 0) gimenez_kernel<0><<<(unsigned)(n_pv * bpp), 256, in_smem ? coef_bytes : 0, st>>>(A, (int)bpp, in_smem);
+  else gimenez_kernel<1><<<(unsigned)(n_pv * bpp), 256, 0, st>>>(A, (int)bpp, 0);
   g_launches.fetch_add(1);
   return cudaGetLastError() == cudaSuccess ? PT_OK : PT_ERR_CUDA;
 }
