@@ -375,7 +375,10 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   const int n_prep = Q.n_rec_blocks + Q.n_axis_blocks + Q.n_order_blocks + Q.n_base_blocks;
   // epoch kernel: interpolated model = blocks of 16 warps that stage the table (n_z doubles of shared memory, two per SM);
   // exact model = single-warp blocks, 24 per SM.  About four units per block so that the ticket counter balances the load.
-  const int e_nt = (mode == 1) ? 512 : 32;
+#ifndef PT_EPOCH_NT
+#define PT_EPOCH_NT 512
+#endif
+  const int e_nt = (mode == 1) ? PT_EPOCH_NT : 32;
   const int64_t e_grid = (int64_t)sm_count() * ((mode == 1) ? 2 : PT_EPOCH_WARPS);
   const size_t e_smem = (mode == 1) ? (size_t)tb->n_z * sizeof(double) : 0;
   if (want_epoch) {
@@ -433,7 +436,7 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
     if (mode == 0) {
       if (dtype == PT_F64) PT_EPOCH_T(0, 32, double); else if (dtype == PT_F32) PT_EPOCH_T(0, 32, float); else PT_EPOCH_T(0, 32, Chi2);
     } else {
-      if (dtype == PT_F64) PT_EPOCH_T(1, 512, double); else if (dtype == PT_F32) PT_EPOCH_T(1, 512, float); else PT_EPOCH_T(1, 512, Chi2);
+      if (dtype == PT_F64) PT_EPOCH_T(1, PT_EPOCH_NT, double); else if (dtype == PT_F32) PT_EPOCH_T(1, PT_EPOCH_NT, float); else PT_EPOCH_T(1, PT_EPOCH_NT, Chi2);
     }
 #undef PT_EPOCH_T
 #undef PT_EPOCH
