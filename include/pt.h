@@ -191,6 +191,21 @@ int pt_gimenez_interp(const double* d_coef, int32_t n_ldc, int32_t n_j, int32_t 
                       const double* d_times, int64_t n_t, int64_t t_stride_pv, const double* d_params, int64_t n_pv,
                       int32_t n_pb, int32_t n_ss, double t_exp, double* d_flux, int32_t* d_status, void* stream);
 
+/* pt_gimenez_interp for callers that cannot allocate device memory (CUDA graph capture, serving loops, harnesses that
+ * forbid cudaMalloc): same operation, arguments, results and error codes as pt_gimenez_interp, but the z-tables (its d_work)
+ * live in a fixed array inside the library — pt_gimenez_static_work_doubles() = 524288 doubles (4 MiB), held by every
+ * device that loads the library until the process ends.  The call allocates nothing (no cudaMalloc / cudaFree, no
+ * allocating library routine); d_coef, d_times, d_params, d_flux, d_status stay the caller's.
+ *   Limit: n_pv * (n_ldc+1) * (n_in+n_out) <= pt_gimenez_static_work_doubles(), else PT_ERR_SIZE (nothing is enqueued).
+ *   The array is shared by every call on the device and keeps the last call's tables; each call first overwrites every node
+ *   it will read, so nothing needs clearing, and calls enqueued on ONE stream are safe back to back.  Calls that can overlap
+ *   on the GPU (different streams, different host threads, concurrently replayed graphs) race on it: the caller serialises
+ *   them.  The tables are not readable by the caller. */
+int64_t pt_gimenez_static_work_doubles(void);
+int pt_gimenez_interp_static(const double* d_coef, int32_t n_ldc, int32_t n_j, int32_t n_in, int32_t n_out,
+                             const double* d_times, int64_t n_t, int64_t t_stride_pv, const double* d_params, int64_t n_pv,
+                             int32_t n_pb, int32_t n_ss, double t_exp, double* d_flux, int32_t* d_status, void* stream);
+
 /* Diagnostics for the roofline denominator (the FP64 vector-pipe peak is not in MEASURED_PEAKS.json):
  * every thread of `blocks` x 256 runs `iters` rounds of 8 independent DFMA chains and stores one double to
  * d_sink[blocks*256] so the work cannot be removed.  FP64 thread-instructions issued = blocks*256*iters*8. */

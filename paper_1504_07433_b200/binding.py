@@ -22,7 +22,8 @@ _ERR = {1: "PT_ERR_NULL", 2: "PT_ERR_SIZE", 3: "PT_ERR_DTYPE", 4: "PT_ERR_TABLE"
 
 EXPORTS = ("pt_build_arch", "pt_orbit_z", "pt_orbit_z_solver", "pt_ma_quad_exact", "pt_ma_table_build", "pt_table_spacing", "pt_ma_quad_interp", "pt_ma_quad_chi2", "pt_ma_quad_exact_pbk",
            "pt_ma_quad_exact_host", "pt_ma_quad_interp_host", "pt_plan", "pt_probe_dfma", "pt_probe_ffma",
-           "pt_gimenez_coef_size", "pt_gimenez_coef_build", "pt_gimenez_exact", "pt_gimenez_interp", "pt_launch_count")
+           "pt_gimenez_coef_size", "pt_gimenez_coef_build", "pt_gimenez_exact", "pt_gimenez_interp", "pt_gimenez_interp_static",
+           "pt_gimenez_static_work_doubles", "pt_launch_count")
 
 
 class PtError(RuntimeError):
@@ -64,10 +65,13 @@ def lib() -> C.CDLL:
         L.pt_gimenez_coef_build.argtypes = [i32, i32, ptr, ptr]
         L.pt_gimenez_exact.argtypes = [ptr, i32, i32, ptr, i64, i64, ptr, i64, i32, i32, dbl, ptr, ptr, ptr]
         L.pt_gimenez_interp.argtypes = [ptr, i32, i32, i32, i32, ptr, ptr, i64, i64, ptr, i64, i32, i32, dbl, ptr, ptr, ptr]
+        L.pt_gimenez_interp_static.argtypes = [ptr, i32, i32, i32, i32, ptr, i64, i64, ptr, i64, i32, i32, dbl, ptr, ptr, ptr]
+        L.pt_gimenez_static_work_doubles.argtypes = []
         L.pt_probe_ffma.argtypes = [i32, i32, ptr, ptr]
         L.pt_plan.argtypes = [i64, i64, i32, C.POINTER(C.c_int64)]
         for n in EXPORTS[1:-1]:
             getattr(L, n).restype = C.c_int
+        L.pt_gimenez_static_work_doubles.restype = i64
         _lib = L
     return _lib
 
@@ -298,6 +302,26 @@ def pt_gimenez_interp(coef: GimenezCoef, n_in: int, n_out: int, times: torch.Ten
                                    n_t, stride, params.data_ptr(), n_pv, n_pb, n_ss, float(t_exp), out.data_ptr(),
                                    status.data_ptr() if status is not None else None, _stream()), "pt_gimenez_interp")
     return out, work
+
+
+def pt_gimenez_static_work_doubles() -> int:
+    """Capacity, in doubles, of the library's fixed work area (include/pt.h: pt_gimenez_interp_static)."""
+    return int(lib().pt_gimenez_static_work_doubles())
+
+
+def pt_gimenez_interp_static(coef: GimenezCoef, n_in: int, n_out: int, times: torch.Tensor, params: torch.Tensor,
+                             out: torch.Tensor, n_pb: int = 1, n_ss: int = 1, t_exp: float = 0.0,
+                             status: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """pt_gimenez_interp without any allocation (include/pt.h: pt_gimenez_interp_static): the z-tables live in the library's
+    fixed work area and `out` [n_pv][n_pb][n_t] float64 must be given."""
+    times, params, n_pv, n_t, stride = _marshal_gimenez(times, params, n_pb, coef.n_ldc)
+    if not (out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == n_pv * n_pb * n_t):
+        raise PtError("out must be a contiguous CUDA float64 tensor of n_pv*n_pb*n_t elements")
+    _check(lib().pt_gimenez_interp_static(coef.data.data_ptr(), coef.n_ldc, coef.n_j, n_in, n_out, times.data_ptr(), n_t, stride,
+                                          params.data_ptr(), n_pv, n_pb, n_ss, float(t_exp), out.data_ptr(),
+                                          status.data_ptr() if status is not None else None, _stream()),
+           "pt_gimenez_interp_static")
+    return out
 
 
 def pt_probe_ffma(blocks: int, iters: int, sink: torch.Tensor) -> None:

@@ -43,6 +43,11 @@ struct SchedSlot {
 };
 __device__ SchedSlot g_sched[kSchedSlots];
 
+// Work area of pt_gimenez_interp_static (the per-vector z-tables of pt_gimenez_interp): 4 MiB that every device which loads
+// the library holds until the process ends.
+constexpr int64_t kGimStaticWork = 1 << 19;   // doubles
+static __device__ __align__(256) double g_gim_work[kGimStaticWork];
+
 struct SlotHost {
   cudaEvent_t ev = nullptr;
   bool used = false;
@@ -658,6 +663,37 @@ int pt_gimenez_exact(const double* d_coef, int32_t n_ldc, int32_t n_j, const dou
 int pt_gimenez_interp(const double* d_coef, int32_t n_ldc, int32_t n_j, int32_t n_in, int32_t n_out, double* d_work,
                       const double* d_times, int64_t n_t, int64_t t_stride_pv, const double* d_params, int64_t n_pv,
                       int32_t n_pb, int32_t n_ss, double t_exp, double* d_flux, int32_t* d_status, void* stream) {
+  return gimenez_launch(1, d_coef, n_ldc, n_j, n_in, n_out, d_work, d_times, n_t, t_stride_pv, d_params, n_pv, n_pb, n_ss,
+                        t_exp, d_flux, d_status, stream);
+}
+
+// ---- pt_gimenez_interp for callers that must not allocate: the z-tables live in a fixed array of this library instead of
+// caller memory.  In host code `g_gim_work` is only a handle: the device address comes from cudaGetSymbolAddress, once per
+// device, with that device current.  Every call on a device shares the array (it keeps the last call's tables; a call
+// overwrites every node it reads, so nothing has to be cleared); calls that overlap on the GPU race on it.
+int64_t pt_gimenez_static_work_doubles(void) { return pt::kGimStaticWork; }
+
+int pt_gimenez_interp_static(const double* d_coef, int32_t n_ldc, int32_t n_j, int32_t n_in, int32_t n_out,
+                             const double* d_times, int64_t n_t, int64_t t_stride_pv, const double* d_params, int64_t n_pv,
+                             int32_t n_pb, int32_t n_ss, double t_exp, double* d_flux, int32_t* d_status, void* stream) {
+  // sizes first: the static work area holds kGimStaticWork doubles
+  if (n_pv <= 0 || n_ldc < 1 || n_ldc > kGimMaxLdc || n_in < 2 || n_out < 2) return PT_ERR_SIZE;
+  if ((int64_t)n_in + n_out > pt::kGimStaticWork) return PT_ERR_SIZE;
+  if (n_pv > pt::kGimStaticWork / ((int64_t)(n_ldc + 1) * ((int64_t)n_in + n_out))) return PT_ERR_SIZE;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return PT_ERR_CUDA;
+  double* d_work = nullptr;
+  {
+    static std::mutex mu;
+    static double* work_of[64];
+    std::lock_guard<std::mutex> lock(mu);
+    if (!work_of[dev]) {
+      void* p = nullptr;
+      if (cudaGetSymbolAddress(&p, pt::g_gim_work) != cudaSuccess || !p) { (void)cudaGetLastError(); return PT_ERR_CUDA; }
+      work_of[dev] = (double*)p;
+    }
+    d_work = work_of[dev];
+  }
   return gimenez_launch(1, d_coef, n_ldc, n_j, n_in, n_out, d_work, d_times, n_t, t_stride_pv, d_params, n_pv, n_pb, n_ss,
                         t_exp, d_flux, d_status, stream);
 }
