@@ -12,8 +12,9 @@
 // front of each of them: epoch j owns the exposures [hi_{j-1}, hi_j) — the gap before its window, written as pure 16-byte
 // streaming stores (no time loads, no arithmetic), and its window, every exposure of which is evaluated.  hi_{-1} = 0 and
 // the last epoch of the row also owns the tail, so the units partition the output exactly and nothing is searched twice.
-// (A batch of epochs writes its ones as ONE run over its whole stretch and then overwrites the windows — same warp, ordered by
-// a __syncwarp — instead of one short run per gap: 4 % more bytes, a tenth of the fill instructions; PT_FILL_THROUGH.)
+// (A batch of epochs writes ones over its whole stretch, windows included, and overwrites the windows — same warp, ordered by
+// a __syncwarp — instead of one short run per gap: 4 % more bytes, a tenth of the fill instructions; PT_FILL_THROUGH.  In the
+// interpolated model the stretch goes out piece by piece, each in front of the round of the evaluation that needs it.)
 // Units are dealt to the blocks of one persistent grid from a ticket counter, rows in the order prep_kernel left (by k̂
 // for the table: neighbouring tickets read neighbouring table rows; heaviest first for the exact model).
 //
@@ -23,7 +24,8 @@
 //     T[ik][j][f])); a sample is then 1 - (G[iz] + fz (G[iz+1] - G[iz])) from shared memory — the same bilinear rule
 //     (S§8(c)-2 step 8) with the k-blend done first.  No per-sample gather from L2 is left.
 //   exact model (MODE 0): a block is a single autonomous warp (no barrier cost, 24 of them per SM).
-//   Inside a unit the warps take batches of up to 32 epochs (lane = epoch: probes, searches), fill the gaps, and pack the
+//   Inside a unit every warp takes an equal run of consecutive epochs, in as few batches of up to 31 epochs as possible
+//   (lane = epoch: probes, searches), fills the gaps, and packs the
 //   in-window exposures of the batch (times n_ss subsamples) densely over the lanes in rounds of 32: pinned subsample time
 //   and phase fold (H1, H2), orbit, in-transit test, basis functions or table lookup, limb-darkening combine;
 //   n_ss > 1: segmented warp-shuffle sum in 64-bit fixed point (order-independent: bit-reproducible), carried across
@@ -42,9 +44,19 @@ namespace pt {
 #define PT_FILL_THROUGH 1     // 1: a batch writes ones over its whole stretch and overwrites the windows (0.737 -> 0.704 ms on configs[3]);
                                // 0: only the gaps are filled, every element is written exactly once
 #endif
-#ifndef PT_STATIC_BATCHES
-#define PT_STATIC_BATCHES 1   // 1: every warp of a block takes a run of consecutive batches, so its stores walk through one
-                              // contiguous piece of the row (configs[3] 0.704 -> 0.682 ms); 0: batches from a counter
+#ifndef PT_FILL_ROUNDS_INTERP
+#define PT_FILL_ROUNDS_INTERP 1   // the stretch of a batch is written piece by piece in front of the rounds of its evaluation
+                                  // (configs[3]: 0.80 ms with the whole stretch first, 0.67 ms piece by piece)
+#endif
+#ifndef PT_FILL_ROUNDS_EXACT
+#define PT_FILL_ROUNDS_EXACT 0     // exact model: the whole stretch in front of the rounds (configs[1] 0.083 vs 0.079 ms)
+#endif
+#ifndef PT_EPOCH_DEPTH
+#define PT_EPOCH_DEPTH 3          // rounds of time loads in flight ahead of the evaluation, interpolated model (1 / 2 / 3: 0.674 / 0.673 / 0.670 ms)
+#endif
+#ifndef PT_EPOCH_FILL_AHEAD
+#define PT_EPOCH_FILL_AHEAD 1      // pieces of ones written ahead of the round being evaluated (1 / 2 / 3 / 4: 0.675 / 0.700 / 0.716 / 0.763 ms:
+                                   // longer bursts of stores from one warp hold up everybody's loads)
 #endif
 #ifndef PT_EPOCH_WARPS
 #define PT_EPOCH_WARPS 24   // single-warp blocks per SM of the exact model's epoch kernel
@@ -182,7 +194,6 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? PT_EPOCH_WARPS : 2)) epoch_ker
   __shared__ double s_off[SS1 ? 1 : kOffTable];
   __shared__ PvRec s_rec;
   __shared__ unsigned long long s_tk;
-  __shared__ int s_next;
   constexpr int nwp = NT / 32;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   EpochWarp& W = s_w[SS1 ? 0 : warp];
@@ -207,7 +218,7 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? PT_EPOCH_WARPS : 2)) epoch_ker
 
   unsigned long long ticket = blockIdx.x;
   while (ticket < n_units) {
-    if (tid == 0) { s_tk = atomicAdd(A.sched + kW_Ticket, 1ULL); s_next = 0; }   // the next ticket: its latency hides behind this unit
+    if (tid == 0) { s_tk = atomicAdd(A.sched + kW_Ticket, 1ULL); }   // the next ticket: its latency hides behind this unit
     const int64_t j = (int64_t)(ticket / (unsigned long long)C);
     const int c = (int)(ticket - (unsigned long long)j * C);
     const int64_t pv = A.order ? (int64_t)__ldg(A.order + j) : j;
@@ -239,6 +250,14 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? PT_EPOCH_WARPS : 2)) epoch_ker
       const uint32_t E0 = (uint32_t)((unsigned long long)c * cnt / (unsigned long long)C);
       const uint32_t E1 = (uint32_t)((unsigned long long)(c + 1) * cnt / (unsigned long long)C);
       const bool use_tb = MODE == 1 && r.use_table;
+      // batches of Be <= 31 epochs (lane = epoch; one more lane looks at the epoch in front of the batch).
+      // Every warp takes an equal run of consecutive epochs — its stores walk through one contiguous piece of the row — cut
+      // into as few batches as possible: a batch costs an exposed load (its probes; the times of a window then hit L1).
+      const uint32_t nE = E1 - E0;
+      const uint32_t nEw = (nE + nwp - 1u) / nwp;
+      const uint32_t wE0 = min(E0 + (uint32_t)warp * nEw, E1), wE1 = min(wE0 + nEw, E1);
+      const uint32_t nS = (nEw + 30u) / 31u;
+      const uint32_t Be = nS ? (nEw + nS - 1u) / nS : 1u;
       if (MODE == 1 && use_tb && E1 > E0) {
         stage_table<NT>(A, r, s_G, pol);
         __syncthreads();
@@ -246,29 +265,9 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? PT_EPOCH_WARPS : 2)) epoch_ker
       const double khat = r.c.khat;
       const bool slow_div = flags & PV_SLOWDIV;
       const double c0 = r.coef[0], c1 = r.coef[1], c2 = r.coef[2];
-      // batches of Be <= 31 epochs (lane = epoch; one more lane looks at the epoch in front of the batch)
-      const uint32_t nE = E1 - E0;
-#ifndef PT_BE_DIV
-#define PT_BE_DIV 5u
-#endif
-      uint32_t Be = (nwp == 1) ? 31u : (nE + PT_BE_DIV * nwp - 1u) / (PT_BE_DIV * nwp);
-      Be = Be < 4u ? 4u : (Be > 31u ? 31u : Be);
-      const int nbat = (int)((nE + Be - 1u) / Be);
       double chi = 0.0;
-#if PT_STATIC_BATCHES
-      // every warp takes a run of consecutive batches: its stores walk through one contiguous piece of the row
-      const int bper = (nbat + nwp - 1) / nwp;
-      const int b_lo = warp * bper, b_hi = min((warp + 1) * bper, nbat);
-      for (int bi = b_lo; bi < b_hi; ++bi) {
-#else
-      for (;;) {
-        int bi = 0;
-        if (lane == 0) bi = atomicAdd(&s_next, 1);
-        bi = __shfl_sync(0xffffffffu, bi, 0);
-        if (bi >= nbat) break;
-#endif
-        const uint32_t first = E0 + (uint32_t)bi * Be;
-        const int m = (int)min(Be, E1 - first);
+      for (uint32_t first = wE0; first < wE1; first += Be) {
+        const int m = (int)min(Be, wE1 - first);
         // lane i < m: epoch first + i; lane m: the epoch in front of the batch (only its hi is used)
         int lo = 0, hi = 0;
         {
@@ -290,13 +289,22 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? PT_EPOCH_WARPS : 2)) epoch_ker
         const int phi0 = __shfl_sync(0xffffffffu, hi, m);
         if (lane == 0) phi = phi0;
 #if PT_FILL_THROUGH
-        // one long run of ones over the whole stretch of the batch, windows included; the evaluation below overwrites the
-        // windows (same warp, ordered by the __syncwarp): a few per cent more bytes, a tenth of the fill instructions
-        if constexpr (!kIsChi2<OutT>) {
-          const int hl = __shfl_sync(0xffffffffu, hi, m - 1);
-          fill_span<V2, OutT>(row, (uint32_t)phi0, (uint32_t)((first + (uint32_t)m == cnt) ? n_t : hl), (OutT)1.0);
-          __syncwarp();
-        }
+        // ones over the whole stretch of the batch, windows included; the evaluation overwrites the windows (same warp, ordered
+        // by a __syncwarp): a few per cent more bytes, a tenth of the fill instructions.  The stretch is written piece by piece
+        // in front of the rounds of the evaluation (`fill_to`), each piece ending with the window of the round's last sample.
+        const int bend = (first + (uint32_t)m == cnt) ? n_t : __shfl_sync(0xffffffffu, hi, m - 1);
+        int filled = phi0;
+        constexpr bool kPerRound = (MODE == 1) ? (PT_FILL_ROUNDS_INTERP != 0) : (PT_FILL_ROUNDS_EXACT != 0);
+        auto fill_to = [&](int need) {
+          if constexpr (!kIsChi2<OutT>) {
+            if (need > filled) {
+              fill_span<V2, OutT>(row, (uint32_t)filled, (uint32_t)need, (OutT)1.0);
+              filled = need;
+              __syncwarp();
+            }
+          }
+        };
+        if (!kPerRound) fill_to(bend);
         (void)phi;
 #else
         for (int i = 0; i < m; ++i) {
@@ -307,6 +315,9 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? PT_EPOCH_WARPS : 2)) epoch_ker
         if constexpr (!kIsChi2<OutT>) {
           if (first + (uint32_t)m == cnt) fill_span<V2, OutT>(row, (uint32_t)__shfl_sync(0xffffffffu, hi, m - 1), (uint32_t)n_t, (OutT)1.0);   // tail of the row
         }
+        const int bend = 0;
+        auto fill_to = [&](int) {};
+        (void)bend;
 #endif
         // in-window exposures of the batch, packed over the lanes
         const int rcnt = lane < m ? hi - lo : 0;
@@ -318,14 +329,20 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? PT_EPOCH_WARPS : 2)) epoch_ker
         }
         const int n_exp = __shfl_sync(0xffffffffu, cum, 31);
         const int ebase = lo - (cum - rcnt);              // exposure x of the batch, if it lies in this lane's range, is e = ebase + x
-        auto exposure_of = [&](int x) -> int {            // the range i with cum[i-1] <= x < cum[i]
+        auto range_of = [&](int x) -> int {               // the range i with cum[i-1] <= x < cum[i]
           int i = 0;
 #pragma unroll
           for (int step = 16; step > 0; step >>= 1) {
             const int cv = __shfl_sync(0xffffffffu, cum, i + step - 1);
             if (cv <= x) i += step;
           }
-          return __shfl_sync(0xffffffffu, ebase, i) + x;
+          return i;
+        };
+        auto exposure_of = [&](int x) -> int { return __shfl_sync(0xffffffffu, ebase, range_of(x)) + x; };
+        // end of the stretch that must hold its ones before the samples up to x_last (uniform) are stored
+        auto stretch_end = [&](int x_last, bool last_round) -> int {
+          if (!kPerRound) return bend;
+          return last_round ? bend : __shfl_sync(0xffffffffu, hi, range_of(x_last));
         };
         auto decrement = [&](double zs) -> double {       // combined decrement of an in-transit sample
           if (MODE == 1 && use_tb) {
@@ -346,7 +363,6 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? PT_EPOCH_WARPS : 2)) epoch_ker
         };
         if (SS1) {
           const int R = (n_exp + 31) >> 5;
-          int e1 = 0; double t1 = 0.0; bool a1 = false;
           auto fetch = [&](int q, int& e, double& t, bool& act) {
             const int x = q * 32 + lane;
             act = x < n_exp;
@@ -360,10 +376,23 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? PT_EPOCH_WARPS : 2)) epoch_ker
               }
             }
           };
-          if (R > 0) fetch(0, e1, t1, a1);
+          // the times of the next kDepth rounds are in flight during this one (under a saturated store stream a load that
+          // misses L1 takes microseconds; most of a window's times were brought into L1 by its probes)
+          constexpr int kDepth = (MODE == 1) ? PT_EPOCH_DEPTH : 1;
+          int eq[kDepth]; double tq[kDepth]; bool aq[kDepth];
+#pragma unroll
+          for (int d = 0; d < kDepth; ++d) {
+            eq[d] = 0; tq[d] = 0.0; aq[d] = false;
+            if (d < R) fetch(d, eq[d], tq[d], aq[d]);
+          }
           for (int q = 0; q < R; ++q) {
-            const int e = e1; const double t = t1; const bool act = a1;
-            if (q + 1 < R) fetch(q + 1, e1, t1, a1);       // the next round's times are in flight during this one
+            const int e = eq[0]; const double t = tq[0]; const bool act = aq[0];
+#pragma unroll
+            for (int d = 0; d + 1 < kDepth; ++d) { eq[d] = eq[d + 1]; tq[d] = tq[d + 1]; aq[d] = aq[d + 1]; }
+            if (q + kDepth < R) fetch(q + kDepth, eq[kDepth - 1], tq[kDepth - 1], aq[kDepth - 1]);
+#if PT_FILL_THROUGH
+            fill_to(stretch_end(min((q + PT_EPOCH_FILL_AHEAD) * 32 - 1, n_exp - 1), q + PT_EPOCH_FILL_AHEAD >= R));
+#endif
             if (act) {
               bool in;
               const double zs = sample_z<OutT>(r, fold_phase(t, r.c.t0, r.c.P, r.c.invP, slow_div), in);
@@ -371,6 +400,7 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? PT_EPOCH_WARPS : 2)) epoch_ker
               if (in || !kIsChi2<OutT>) emit1<OutT>(A, row, (uint32_t)e, dec, chi);
             }
           }
+          fill_to(bend);                                   // a batch without a single in-window exposure
         } else {
           // supersampled: items y = x n_ss + s, 32 per round; segmented fixed-point sum per exposure, carried in W.acc
           const long long n_items = (long long)n_exp * n_ss;
@@ -382,6 +412,13 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? PT_EPOCH_WARPS : 2)) epoch_ker
             const bool act = x < n_exp;
             const int e = exposure_of(act ? x : n_exp - 1);
             PT_CHECK(e >= 0 && e < n_t && sub >= 0 && sub < n_ss);
+#if PT_FILL_THROUGH
+            {
+              const long long yl = y0 + 31;
+              const int xl = (n_items < 0x7fffffffLL) ? (int)((uint32_t)yl / (uint32_t)n_ss) : (int)(yl / n_ss);
+              fill_to(stretch_end(min(xl, n_exp - 1), y0 + 32 >= n_items));
+            }
+#endif
             long long fx = 0;
             if (act) {
               const double t = ldg_keep(A.times + e, pol);
@@ -409,6 +446,7 @@ __global__ void __launch_bounds__(NT, (NT == 32 ? PT_EPOCH_WARPS : 2)) epoch_ker
             }
             __syncwarp();
           }
+          fill_to(bend);
         }
       }
       if constexpr (kIsChi2<OutT>) {
