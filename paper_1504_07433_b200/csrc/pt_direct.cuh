@@ -19,6 +19,9 @@
 
 namespace pt {
 
+#ifndef PT_DIRECT_ONE_COPY
+#define PT_DIRECT_ONE_COPY 1
+#endif
 #ifndef PT_DIRECT_BLOCKS
 #define PT_DIRECT_BLOCKS 3
 #endif
@@ -89,8 +92,19 @@ __global__ void __launch_bounds__(kThreads, PT_DIRECT_BLOCKS) direct_kernel(cons
         for (int e = 2 * lane; e < n2; e += 64) {
           const double2 tv = __ldg((const double2*)(tb + e));
           V2T o;
+#if PT_DIRECT_ONE_COPY
+          // one copy of the evaluation in the instruction stream, run twice (the loop is kept rolled on purpose)
+          double ta = tv.x;
+          o.y = (OutT)0;
+#pragma unroll 1
+          for (int k = 0; k < 2; ++k) {
+            const OutT v = flux_of(ta);
+            o.x = o.y; o.y = v; ta = tv.y;
+          }
+#else
           o.x = flux_of(tv.x);
           o.y = flux_of(tv.y);
+#endif
           PT_ST((V2T*)(ob + e), o);
         }
         if ((n_e & 1) && lane == 0) PT_ST(ob + n2, flux_of(__ldg(tb + n2)));
