@@ -42,6 +42,7 @@ __global__ void __launch_bounds__(kThreads, PT_DIRECT_BLOCKS) direct_kernel(cons
   WarpState& ws = s_ws[warp];
   const unsigned long long gw = (unsigned long long)blockIdx.x * kWarpsPerBlock + warp, nw = (unsigned long long)gridDim.x * kWarpsPerBlock;
   const int tpp = A.tiles_per_pv;
+  if (A.prep) asm volatile("griddepcontrol.wait;" ::: "memory");   // prep_kernel's records are complete
   int64_t last_pv = -1;
   unsigned long long tile = gw;
   while (tile < (unsigned long long)A.n_tiles) {
@@ -89,8 +90,19 @@ __global__ void __launch_bounds__(kThreads, PT_DIRECT_BLOCKS) direct_kernel(cons
       if (V == 2) {
         typedef typename Vec2<OutT>::type V2T;
         const int n2 = n_e & ~1;
-        for (int e = 2 * lane; e < n2; e += 64) {
-          const double2 tv = __ldg((const double2*)(tb + e));
+        V2T ones; ones.x = (OutT)1.0; ones.y = (OutT)1.0;
+        double2 nx = make_double2(0.0, 0.0);
+        if (2 * lane < n2) nx = __ldg((const double2*)(tb + 2 * lane));
+        for (int e0 = 0; e0 < n2; e0 += 64) {
+          const int e = e0 + 2 * lane;
+          const double2 tv = nx;
+          if (e + 64 < n2) nx = __ldg((const double2*)(tb + e + 64));      // the next round's times are in flight
+          const bool any = (e < n2) && (in_window2(tv.x, invP, w_c0, w_half) || in_window2(tv.y, invP, w_c0, w_half));
+          if (!__any_sync(0xffffffffu, any)) {                             // nothing of this round can be in transit
+            if (e < n2) PT_ST((V2T*)(ob + e), ones);
+            continue;
+          }
+          if (e >= n2) continue;
           V2T o;
 #if PT_DIRECT_ONE_COPY
           // one copy of the evaluation in the instruction stream, run twice (the loop is kept rolled on purpose)

@@ -14,6 +14,11 @@
 #include "pt_direct.cuh"
 #include "pt_gimenez.cuh"
 
+#ifndef PT_REC_MIN_TILES
+#define PT_REC_MIN_TILES 2   // tiles per row from which prep_kernel computes the records once (dense 4096 x 4096, six tiles per
+                             // row: 0.510 -> 0.458 ms against a threshold of eight)
+#endif
+
 namespace pt {
 
 static std::atomic<int64_t> g_launches{0};
@@ -341,12 +346,12 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   if (!slot) return PT_ERR_CUDA;
   A.sched = slot->w;
   // What prep_kernel is asked to leave in the slot (pt_flux.cuh):
-  //   records  single passband, at most kPvCacheMax parameter vectors, many tiles each (the per-tile setup is 15 % of the
-  //            flux kernel's instructions on configs[1] when done per tile)
+  //   records  single passband, at most kPvCacheMax parameter vectors, at least two tiles each (the per-tile setup is 15 % of
+  //            the flux kernel's instructions on configs[1] when done per tile, 18 % of the direct kernel's time on `dense`)
   //   axis     one shared time axis of a problem large enough for the extra launch to pay: is it ascending?
   //   order    global tile counter: heaviest rows first (mode 2), or rows by k̂ for the interpolated model
   //   baseline fused likelihood
-  const bool want_rec = n_pb == 1 && pb_view < 0 && n_pv <= kPvCacheMax && A.n_tiles >= 8 * n_pv &&
+  const bool want_rec = n_pb == 1 && pb_view < 0 && n_pv <= kPvCacheMax && A.n_tiles >= PT_REC_MIN_TILES * n_pv &&
                         (double)n_pv * (double)n_t >= 65536.0;   // a small problem does not pay for the extra launch
   const bool want_axis = t_stride_pv == 0 && n_t >= 2048 && (double)n_pv * (double)n_t >= (double)PT_RANGE_MIN;
   // epoch kernel: one passband on one shared axis that prep_kernel checks; it does the whole launch if the axis is ascending,
@@ -356,15 +361,7 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   const bool want_order = n_pv <= kPvCacheMax && n_pv >= 2 &&
                           (want_epoch || plan.mode == 2 || (mode == 1 && plan.mode == 0 && A.n_tiles >= 4 * (int64_t)grid.x * kWarpsPerBlock));
   // direct kernel: the fp32 variant where there are no epochs to look for (per-row times, or a small problem)
-  if (f32a && n_ss == 1 && !want_epoch) {
-    const bool dv2 = (n_t % 2 == 0) && (t_stride_pv % 2 == 0) && (reinterpret_cast<uintptr_t>(d_times) % 16 == 0) &&
-                     (reinterpret_cast<uintptr_t>(d_flux) % 16 == 0);
-    if (dv2) direct_kernel<2, float, 3><<<grid, kThreads, 0, st>>>(A); else direct_kernel<1, float, 3><<<grid, kThreads, 0, st>>>(A);
-    g_launches.fetch_add(1);
-    const cudaError_t derr = cudaGetLastError();
-    slot_release(ticket, st);
-    return derr == cudaSuccess ? PT_OK : PT_ERR_CUDA;
-  }
+  const bool use_direct = f32a && n_ss == 1 && !want_epoch;
   PrepArgs Q{};
   if (want_rec || want_epoch) { Q.rec = slot->pv; Q.n_rec_blocks = (int)((n_pv + kWarpsPerBlock - 1) / kWarpsPerBlock); }
   if (want_axis) { int nb = (int)((n_t + 8 * kThreads - 1) / (8 * kThreads)); Q.n_axis_blocks = nb > 64 ? 64 : nb; }
@@ -419,6 +416,14 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = grid; cfg.blockDim = dim3(kThreads); cfg.dynamicSmemBytes = 0; cfg.stream = st;
   cfg.attrs = pdl_attr; cfg.numAttrs = A.prep ? 1 : 0;
+  if (use_direct) {
+    const bool dv2 = v2 && reinterpret_cast<uintptr_t>(d_flux) % 16 == 0;
+    const cudaError_t d_err = dv2 ? cudaLaunchKernelEx(&cfg, direct_kernel<2, float, 3>, A) : cudaLaunchKernelEx(&cfg, direct_kernel<1, float, 3>, A);
+    g_launches.fetch_add(1);
+    const cudaError_t err2 = cudaGetLastError();
+    slot_release(ticket, st);
+    return (d_err == cudaSuccess && err2 == cudaSuccess) ? PT_OK : PT_ERR_CUDA;
+  }
   if (want_epoch) {
     cudaLaunchConfig_t ecfg = cfg;
     ecfg.gridDim = dim3((unsigned)e_grid);
