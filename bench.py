@@ -41,14 +41,14 @@ FP64_LANES_PER_SM, FP32_LANES_PER_SM, N_SM = 64, 128, 148
 #   dram       dram__bytes_read.sum + dram__bytes_write.sum (a kernel's output that is still in L2 when the capture ends
 #              is not in its figure: configs[1] writes 30.7 MB < 126 MB L2)
 CAPTURES = {
-    "exact_config2": {"fp64_inst": 319160231.0, "pipe_pct": 47.7, "dram": 565760.0, "kernel": "epoch_kernel<0,32,1,0,double>", "ncu_us": 76.4},
-    "scaled": {"fp64_inst": 1995302341.0, "pipe_pct": 57.5, "dram": 161722624.0, "kernel": "epoch_kernel<0,32,1,0,double>", "ncu_us": 342.3},
-    "dense": {"fp64_inst": 4769696118.0, "pipe_pct": 60.7, "dram": 220917504.0, "kernel": "flux_kernel<0,2,1,1,double>", "ncu_us": 520.9},
-    "dense_f32": {"fp64_inst": 733535282.0, "pipe_pct": 13.9, "dram": 172158976.0, "kernel": "direct_kernel<2,float,3>", "ncu_us": 375.5, "fp32_inst": 2235571216.0},
-    "interp_f32": {"fp64_inst": 713357450.0, "pipe_pct": 9.8, "dram": 3287872416.0, "kernel": "epoch_kernel<1,512,1,1,double>", "ncu_us": 652.2},
-    "interp_f64": {"fp64_inst": 713357450.0, "pipe_pct": 9.4, "dram": 3305792920.0, "kernel": "epoch_kernel<1,512,1,1,double>", "ncu_us": 681.1},
-    "config3": {"fp64_inst": 64586338.0, "pipe_pct": 12.2, "dram": 1600768.0, "kernel": "flux_kernel<0,2,0,1,double>", "ncu_us": 52.6},
-    "config5": {"fp64_inst": 5119584261.0, "pipe_pct": 61.3, "dram": 221947136.0, "kernel": "flux_kernel<0,2,1,1,double>", "ncu_us": 563.6},
+    "exact_config2": {"fp64_inst": 319160231.0, "pipe_pct": 48.5, "dram": 551680.0, "kernel": "epoch_kernel<0,32,1,0,double>", "ncu_us": 71.5},
+    "scaled": {"fp64_inst": 1995302341.0, "pipe_pct": 58.9, "dram": 159538688.0, "kernel": "epoch_kernel<0,32,1,0,double>", "ncu_us": 329.6},
+    "dense": {"fp64_inst": 4348782966.0, "pipe_pct": 64.2, "dram": 222173184.0, "kernel": "flux_kernel<0,2,1,1,double>", "ncu_us": 444.7},
+    "dense_f32": {"fp64_inst": 344954141.0, "pipe_pct": 11.6, "dram": 172672256.0, "kernel": "direct_kernel<2,float,3>", "ncu_us": 245.5, "fp32_inst": 2231589904.0},
+    "interp_f32": {"fp64_inst": 710701664.0, "pipe_pct": 7.7, "dram": 3294375512.0, "kernel": "epoch_kernel<1,512,1,1,double>", "ncu_us": 636.6},
+    "interp_f64": {"fp64_inst": 710701664.0, "pipe_pct": 7.4, "dram": 3320690688.0, "kernel": "epoch_kernel<1,512,1,1,double>", "ncu_us": 658.5},
+    "config3": {"fp64_inst": 64586338.0, "pipe_pct": 11.8, "dram": 1892352.0, "kernel": "flux_kernel<0,2,0,1,double>", "ncu_us": 51.7},
+    "config5": {"fp64_inst": 4698671109.0, "pipe_pct": 64.3, "dram": 222058752.0, "kernel": "flux_kernel<0,2,1,1,double>", "ncu_us": 478.1},
 }
 CAPTURE_SOURCE = "profiles/r2_ncu_*.md (ncu --set full + sass op counters, one launch of the same workload)"
 
