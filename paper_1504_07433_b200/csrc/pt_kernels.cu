@@ -361,7 +361,11 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   const bool want_order = n_pv <= kPvCacheMax && n_pv >= 2 &&
                           (want_epoch || plan.mode == 2 || (mode == 1 && plan.mode == 0 && A.n_tiles >= 4 * (int64_t)grid.x * kWarpsPerBlock));
   // direct kernel: the fp32 variant where there are no epochs to look for (per-row times, or a small problem)
-  const bool use_direct = f32a && n_ss == 1 && !want_epoch;
+#ifndef PT_DIRECT_F64
+#define PT_DIRECT_F64 0
+#endif
+  const bool direct64 = PT_DIRECT_F64 && dtype == PT_F64 && mode == 0 && n_pb == 1 && pb_view < 0 && t_stride_pv != 0;
+  const bool use_direct = (f32a || direct64) && n_ss == 1 && !want_epoch;
   PrepArgs Q{};
   if (want_rec || want_epoch) { Q.rec = slot->pv; Q.n_rec_blocks = (int)((n_pv + kWarpsPerBlock - 1) / kWarpsPerBlock); }
   if (want_axis) { int nb = (int)((n_t + 8 * kThreads - 1) / (8 * kThreads)); Q.n_axis_blocks = nb > 64 ? 64 : nb; }
@@ -418,7 +422,9 @@ static int launch_flux(int mode, const pt_table* tb, const double* d_times, int6
   cfg.attrs = pdl_attr; cfg.numAttrs = A.prep ? 1 : 0;
   if (use_direct) {
     const bool dv2 = v2 && reinterpret_cast<uintptr_t>(d_flux) % 16 == 0;
-    const cudaError_t d_err = dv2 ? cudaLaunchKernelEx(&cfg, direct_kernel<2, float, 3>, A) : cudaLaunchKernelEx(&cfg, direct_kernel<1, float, 3>, A);
+    cudaError_t d_err;
+    if (direct64) d_err = dv2 ? cudaLaunchKernelEx(&cfg, direct_kernel<2, double, 0>, A) : cudaLaunchKernelEx(&cfg, direct_kernel<1, double, 0>, A);
+    else d_err = dv2 ? cudaLaunchKernelEx(&cfg, direct_kernel<2, float, 3>, A) : cudaLaunchKernelEx(&cfg, direct_kernel<1, float, 3>, A);
     g_launches.fetch_add(1);
     const cudaError_t err2 = cudaGetLastError();
     slot_release(ticket, st);

@@ -290,6 +290,37 @@ def test_fp32_arith_dense_eccentric_and_shared_axis(pt, oracle):
     assert (f == 1.0).mean() > 0.9                       # out of transit: exactly 1
 
 
+@pytest.mark.parametrize("n_pv,n_t,kind", [(300, 100, "dense"), (64, 3000, "dense"), (40, 3001, "dense"), (7, 40000, "sparse"),
+                                           (33, 2049, "sparse"), (3, 1, "dense")])
+def test_direct_kernel_shapes(pt, oracle, n_pv, n_t, kind):
+    """The direct kernel (fp32 variant, per-row times, n_ss = 1): one tile per row (records per tile) and several (records from
+    prep_kernel), odd row lengths (no 16-byte loads), rows dense and sparse in transits (full and ragged list rounds, passes
+    that leave a remainder), a bad row and a row the rule keeps in fp64 arithmetic — every element written, gate 2e-6."""
+    if kind == "dense":
+        w = inputs.dense_transit(n_pv=n_pv, n_t=n_t)
+        times, params = w.times, w.params
+    else:
+        w = inputs.config2(n_pv=n_pv, n_t=n_t)
+        rng = np.random.default_rng(n_t)
+        times = np.ascontiguousarray(w.times[None, :] + rng.uniform(0.0, 0.01, (n_pv, 1)))
+        params = w.params.copy()
+    params = params.copy()
+    if n_pv > 2:
+        params[1, 1] = -1.0                  # bad row: NaN
+        params[2, 6] = 0.75                  # k > 0.7: the rule keeps this row in fp64 arithmetic (f32_ok)
+    out = torch.full((n_pv, 1, n_t), float("nan"), dtype=torch.float32, device="cuda")
+    st = torch.zeros(2, dtype=torch.int32, device="cuda")
+    pt.pt_ma_quad_exact(dev(times), dev(params), 1, 1, 0.0, out=out, status=st)
+    torch.cuda.synchronize()
+    f = out.cpu().numpy().astype(np.float64)
+    r = oracle.ma_quad_exact(times, params, 1, 1, 0.0, prec="f64")
+    assert np.array_equal(np.isnan(f), np.isnan(r))
+    ok = ~np.isnan(r)
+    assert np.abs(f[ok] - r[ok]).max() <= TOL32
+    if n_pv > 2:
+        assert np.all(np.isnan(f[1])) and st.cpu().tolist() == [pt.PT_ST_BAD_PARAM, 1]
+
+
 # ------------------------------------------------------------------------------------------- table + interpolated path
 def _table_cfg(small=True):
     return dict(k_min=0.05, k_max=0.25, n_k=41, z_max=1.25, n_z=1251) if small else inputs.config4(1, 1).table
