@@ -44,7 +44,7 @@ CAPTURES = {
     "exact_config2": {"fp64_inst": 319160231.0, "pipe_pct": 48.5, "dram": 551680.0, "kernel": "epoch_kernel<0,32,1,0,double>", "ncu_us": 71.5},
     "scaled": {"fp64_inst": 1995302341.0, "pipe_pct": 58.9, "dram": 159538688.0, "kernel": "epoch_kernel<0,32,1,0,double>", "ncu_us": 329.6},
     "dense": {"fp64_inst": 4348782966.0, "pipe_pct": 64.2, "dram": 222173184.0, "kernel": "flux_kernel<0,2,1,1,double>", "ncu_us": 444.7},
-    "dense_f32": {"fp64_inst": 344954141.0, "pipe_pct": 11.6, "dram": 172672256.0, "kernel": "direct_kernel<2,float,3>", "ncu_us": 245.5, "fp32_inst": 2231589904.0},
+    "dense_f32": {"fp64_inst": 311909426.0, "pipe_pct": 9.3, "dram": 173787136.0, "kernel": "direct_kernel<2,float,3>", "ncu_us": 268.4, "fp32_inst": 2231589904.0},
     "interp_f32": {"fp64_inst": 710701664.0, "pipe_pct": 7.7, "dram": 3294375512.0, "kernel": "epoch_kernel<1,512,1,1,double>", "ncu_us": 636.6},
     "interp_f64": {"fp64_inst": 710701664.0, "pipe_pct": 7.4, "dram": 3320690688.0, "kernel": "epoch_kernel<1,512,1,1,double>", "ncu_us": 658.5},
     "config3": {"fp64_inst": 64586338.0, "pipe_pct": 11.8, "dram": 1892352.0, "kernel": "flux_kernel<0,2,0,1,double>", "ncu_us": 51.7},
