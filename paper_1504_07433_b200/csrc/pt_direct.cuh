@@ -138,6 +138,7 @@ __global__ void __launch_bounds__(kThreads, PT_DIRECT_BLOCKS) direct_kernel(cons
             n_list += __popc(bx);
           }
         }
+        PT_CHECK(n_list <= kDirectList);
         __syncwarp();
         // ---- pass 2: full rounds; everything at the end of the tile
         const bool last = s1 == n_e;
