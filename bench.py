@@ -315,6 +315,22 @@ def run_ours(args):
                                           "note": "same algorithmic count as fp64 against the FP32 pipe; the phase fold stays fp64"}
         extra["dense"]["fp32_store_only"] = {"value": wd.n_eval / t_d32s, "unit": UNIT, "ms": t_d32s * 1e3}
         del dt_, dp_, do, do32
+        # the opposite regime for the same two kernels: per-row axes that are sparse in transits (configs[1]'s population x 7,
+        # every row on its own copy of the axis, n_ss = 1): the direct kernel must not lose to the general one there
+        wsp = inputs.config2(n_pv=448)
+        rng_sp = np.random.default_rng(5)
+        st_ = to_dev(wsp.times[None, :] + rng_sp.uniform(0.0, 0.01, (wsp.n_pv, 1)))
+        sp_ = to_dev(wsp.params)
+        so64 = torch.empty((wsp.n_pv, 1, wsp.n_t), dtype=torch.float64, device=dev)
+        so32 = torch.empty((wsp.n_pv, 1, wsp.n_t), dtype=torch.float32, device=dev)
+        t_s64 = _time_steps(lambda: pt.pt_ma_quad_exact(st_, sp_, 1, 1, 0.0, out=so64), 10, 3, flush, 1) / 10
+        t_s32 = _time_steps(lambda: pt.pt_ma_quad_exact(st_, sp_, 1, 1, 0.0, out=so32), 10, 3, flush, 1) / 10
+        n_sp = wsp.n_pv * wsp.n_t
+        extra["dense"]["sparse_rows"] = {"workload": "448 pv x 60000 per-pv times (configs[1] population, own axis per row), n_ss = 1",
+                                         "fp64": {"value": n_sp / t_s64, "unit": UNIT, "ms": t_s64 * 1e3, "kernel": "flux_kernel (general)"},
+                                         "fp32_variant": {"value": n_sp / t_s32, "unit": UNIT, "ms": t_s32 * 1e3, "kernel": "direct_kernel",
+                                                          "speedup_vs_fp64": t_s64 / t_s32}}
+        del st_, sp_, so64, so32
     if rank == 0 and "interp" in sections:
         # -------------------------------------------------------------- configs[3]: table build + interpolated path
         wi = inputs.config4()
